@@ -1,0 +1,134 @@
+/* fd6.h — C ABI of libfd6: the hot path of arXiv 1707.08900 on one B200 (sm_100a).
+ *
+ * One 2N-storage RK3 step of isothermal compressible hydrodynamics,
+ *     D ln(rho)/Dt = -div u                                              (Eq. 1)
+ *     D u/Dt = -cs^2 grad ln(rho) + nu (lap u + 1/3 grad div u + 2 S.grad ln(rho))   (Eq. 2-3; f = 0)
+ * on a periodic nx*ny*nz grid with cubic cells of size dx, sixth-order central differences
+ * (Eq. 6-8), in one of the paper's two stencil paths:
+ *     FD_PATH_55  single fused pass per substep, mixed derivatives by Eq. 8   (Alg. 2)
+ *     FD_PATH_19  two passes per substep, grad(div u) by Eq. 6 applied twice  (Alg. 3, Eq. 14-18)
+ * and the update  w <- alpha_s w + dt*rhs ; F <- F + beta_s w,  s = 1..3, alpha_1 = 0   (Eq. 10)
+ * with Williamson's coefficients alpha = (0,-5/9,-153/128), beta = (1/3,15/16,8/15) (reading G2).
+ *
+ * Conventions for every call
+ *   - Caller arrays are dense, no ghost zone, x fastest: element (i,j,k) at i + nx*(j + ny*k); one array per
+ *     field (structure of arrays); field order ln(rho), u_x, u_y, u_z; element type float
+ *     (FD_F32) or double (FD_F64) as given to fd_create; nx*ny*nz elements each.
+ *   - `where` says where the caller's pointers live: FD_HOST (pageable or pinned host memory; the call copies
+ *     through the context's stream) or FD_DEVICE (device memory of the context's device).
+ *   - Ownership: the caller owns its arrays; the context owns all device state (two ghost-padded copies of the
+ *     four fields, four dense w arrays, one ghost-padded div array once FD_PATH_19 is selected).  w is scratch
+ *     between steps: fd_load, fd_store(FD_HOST) and fd_rhs overwrite it (legal because alpha_1 = 0).
+ *   - Work is enqueued on the context's stream (fd_set_stream; default: the legacy default stream).  Calls with
+ *     FD_HOST pointers return after their copies completed; fd_rk3_step and calls with FD_DEVICE pointers may
+ *     return before the work finished: use fd_sync or the stream.
+ *   - Every function returns FD_OK or an error code, never throws, never aborts; fd_last_error() gives a
+ *     thread-local message for the last failure.  There is no CPU fallback: without a CUDA device fd_create
+ *     fails with FD_ECUDA.
+ *   - A context is not thread-safe; distinct contexts are independent.
+ */
+#ifndef FD6_H
+#define FD6_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fd_ctx fd_ctx; /* opaque, owned by the library */
+
+enum { FD_F32 = 0, FD_F64 = 1 };          /* dtype */
+enum { FD_PATH_55 = 0, FD_PATH_19 = 1 };  /* stencil path */
+enum { FD_HOST = 0, FD_DEVICE = 1 };      /* where caller pointers live */
+enum { FD_OK = 0, FD_EINVAL = 1, FD_ENOMEM = 2, FD_ECUDA = 3, FD_EUNSUPPORTED = 4 };
+
+/* Kernel implementations of the derivative/update step (fd_set_variant).  Both compute the same path;
+ * FD_VARIANT_AUTO picks the fastest one that supports the grid. */
+enum {
+    FD_VARIANT_AUTO = 0,
+    FD_VARIANT_DIRECT = 1, /* one thread per cell, neighbours through L1/L2 (simple, any supported size)      */
+    FD_VARIANT_TILED = 2   /* TMA-staged xy tiles in shared memory, register sliding window along z            */
+};
+
+/* Kernel ids for fd_get_profile. */
+enum {
+    FD_K_PACK = 0,    /* dense -> padded interior */
+    FD_K_UNPACK = 1,  /* padded interior -> dense                         (a0)             */
+    FD_K_HALO_X = 2,  /* periodic ghost fill, x faces                     (a1, a7)         */
+    FD_K_HALO_YZ = 3, /* periodic ghost fill, y/z faces and all edges     (a1, a7)         */
+    FD_K_FUSED55 = 4, /* Eq. 6-8 + Eq. 1-3 + Eq. 10, one pass             (a2-a4)          */
+    FD_K_PASS1 = 5,   /* 19-pt pass 1: div u, partial update Eq. 14-16    (a6)             */
+    FD_K_PASS2 = 6,   /* 19-pt pass 2: grad div by Eq. 6, Eq. 17-18       (a8)             */
+    FD_K_COUNT = 7
+};
+
+/* Device-memory hooks.  alloc returns a device pointer aligned to >= 256 bytes or NULL; `stream` is the
+ * context's stream handle (a cudaStream_t passed as void*).  Installed process-wide; a context keeps the pair
+ * that was installed when it was created.  Passing NULLs restores cudaMalloc/cudaFree. */
+typedef void* (*fd_alloc_fn)(size_t bytes, void* stream, void* user);
+typedef void (*fd_free_fn)(void* ptr, void* user);
+int fd_set_allocator(fd_alloc_fn alloc, fd_free_fn release, void* user);
+
+/* Create a context for an nx*ny*nz periodic grid, cell size dx (= dy = dz), viscosity nu, sound speed cs.
+ * FD_EINVAL: out == NULL, any n < 8, dx <= 0, nu < 0, cs < 0, non-finite parameter, bad dtype.
+ * FD_EUNSUPPORTED: nx % 4 != 0.  FD_ENOMEM / FD_ECUDA: allocation or CUDA failure (message in fd_last_error).
+ * The fields are zero (a uniform state at rest) until fd_load. */
+int fd_create(fd_ctx** out, int nx, int ny, int nz, double dx, double nu, double cs, int dtype);
+
+/* Select the stencil path (default FD_PATH_55) / kernel variant (default FD_VARIANT_AUTO) / stream.
+ * fd_set_path(FD_PATH_19) allocates the div array on first use.  FD_EUNSUPPORTED if the variant cannot run this
+ * grid.  `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream). */
+int fd_set_path(fd_ctx* ctx, int path);
+int fd_set_variant(fd_ctx* ctx, int variant);
+int fd_set_stream(fd_ctx* ctx, void* cuda_stream);
+
+/* Copy the caller's four fields in (and fill the ghost zones) / copy the current fields out. */
+int fd_load(fd_ctx* ctx, const void* lnrho, const void* ux, const void* uy, const void* uz, int where);
+int fd_store(fd_ctx* ctx, void* lnrho, void* ux, void* uy, void* uz, int where);
+
+/* Right-hand side of Eq. 1-3 of the current state with the selected path, into the caller's arrays.  The
+ * state is not changed. */
+int fd_rhs(fd_ctx* ctx, void* d_lnrho, void* d_ux, void* d_uy, void* d_uz, int where);
+
+/* Advance nsteps full RK3 steps (3 substeps each) of size dt.  FD_EINVAL: nsteps < 0 or dt not finite. */
+int fd_rk3_step(fd_ctx* ctx, double dt, int nsteps);
+
+/* Block until everything enqueued by this context has finished; returns FD_ECUDA if a kernel faulted. */
+int fd_sync(fd_ctx* ctx);
+
+/* Release the context and its device memory.  fd_destroy(NULL) is FD_OK. */
+int fd_destroy(fd_ctx* ctx);
+
+/* Message of the last failing call on this thread ("" if none); static thread-local storage. */
+const char* fd_last_error(void);
+
+/* Introspection (read-only). */
+typedef struct fd_info {
+    int nx, ny, nz, dtype, path, variant; /* variant: the one AUTO resolved to            */
+    int pitch_x, pitch_y, pitch_z;        /* padded array extents in elements             */
+    int ghost_x, ghost_y, ghost_z;        /* offset of cell (0,0,0) inside a padded array */
+    size_t field_stride;                  /* elements between consecutive padded fields   */
+    size_t device_bytes;                  /* device memory owned by the context           */
+} fd_info;
+int fd_get_info(const fd_ctx* ctx, fd_info* out);
+
+/* Number of kernels this context has launched since creation (every kernel of the library counts). */
+unsigned long long fd_kernel_launches(const fd_ctx* ctx);
+
+/* Per-kernel device timing: with profiling on, every launch is bracketed by CUDA events on the context's
+ * stream.  fd_get_profile synchronises, then returns the accumulated device milliseconds and launch count of
+ * kernel `kernel_id` since the last fd_reset_profile. */
+int fd_set_profiling(fd_ctx* ctx, int on);
+int fd_get_profile(fd_ctx* ctx, int kernel_id, double* total_ms, unsigned long long* launches);
+int fd_reset_profile(fd_ctx* ctx);
+
+/* Test hooks: overwrite the w arrays / every ghost cell of both field copies with a quiet NaN, to prove that
+ * neither stale w (alpha_1 = 0) nor stale ghosts can reach a result. */
+int fd_debug_poison_w(fd_ctx* ctx);
+int fd_debug_poison_ghosts(fd_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FD6_H */

@@ -1,0 +1,599 @@
+// fd6.cu — the C ABI of libfd6 (include/fd6.h): context, HBM layout, launch sequencing.
+// Every step of the path runs in the kernels of fd6_kernels_*.cuh; this file only allocates, orders
+// launches on the context's stream and swaps pointers.
+#include "../../include/fd6.h"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "fd6_common.cuh"
+#include "fd6_kernels_direct.cuh"
+#include "fd6_kernels_tiled.cuh"
+
+using namespace fd6;
+
+// ------------------------------------------------------------------------------------------------
+// errors
+// ------------------------------------------------------------------------------------------------
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define FD_CUDA(expr)                                                                                      \
+    do {                                                                                                   \
+        cudaError_t e__ = (expr);                                                                          \
+        if (e__ != cudaSuccess) return fail(FD_ECUDA, "%s: %s (%s:%d)", #expr, cudaGetErrorString(e__), __FILE__, __LINE__); \
+    } while (0)
+
+// ------------------------------------------------------------------------------------------------
+// allocator hooks
+// ------------------------------------------------------------------------------------------------
+static fd_alloc_fn g_alloc = nullptr;
+static fd_free_fn g_free = nullptr;
+static void* g_alloc_user = nullptr;
+
+extern "C" int fd_set_allocator(fd_alloc_fn alloc, fd_free_fn release, void* user) {
+    if ((alloc == nullptr) != (release == nullptr)) return fail(FD_EINVAL, "fd_set_allocator: give both hooks or neither");
+    g_alloc = alloc;
+    g_free = release;
+    g_alloc_user = user;
+    return FD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// context
+// ------------------------------------------------------------------------------------------------
+struct ProfRec {
+    int id;
+    cudaEvent_t a, b;
+};
+
+struct fd_ctx {
+    Geom g{};
+    int dtype = FD_F32, path = FD_PATH_55, variant_req = FD_VARIANT_AUTO, variant = FD_VARIANT_DIRECT;
+    double dx = 0, nu = 0, cs = 0;
+    size_t esize = 4;
+    cudaStream_t stream = nullptr;
+    void* F[2] = {nullptr, nullptr};  // two ghost-padded copies of the four fields (read / write)
+    void* W = nullptr;                // four dense w arrays
+    void* Div = nullptr;              // ghost-padded div u (19-point path only)
+    int cur = 0;                      // F[cur] holds the current state with valid ghosts
+    size_t bytes = 0;
+    fd_alloc_fn alloc = nullptr;
+    fd_free_fn release = nullptr;
+    void* alloc_user = nullptr;
+    unsigned long long launches = 0;
+    bool profiling = false;
+    std::vector<ProfRec> pending;
+    std::vector<cudaEvent_t> pool;
+    double prof_ms[FD_K_COUNT] = {};
+    unsigned long long prof_n[FD_K_COUNT] = {};
+    TiledState tiled;  // tensor maps etc. of the tiled variant
+};
+
+static int ctx_alloc(fd_ctx* c, void** p, size_t bytes) {
+    *p = nullptr;
+    if (c->alloc) {
+        *p = c->alloc(bytes, (void*)c->stream, c->alloc_user);
+        if (!*p) return fail(FD_ENOMEM, "allocator hook returned NULL for %zu bytes", bytes);
+    } else {
+        cudaError_t e = cudaMalloc(p, bytes);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            return fail(e == cudaErrorMemoryAllocation ? FD_ENOMEM : FD_ECUDA, "cudaMalloc(%zu): %s", bytes, cudaGetErrorString(e));
+        }
+    }
+    c->bytes += bytes;
+    return FD_OK;
+}
+
+static void ctx_free(fd_ctx* c, void* p) {
+    if (!p) return;
+    if (c->release)
+        c->release(p, c->alloc_user);
+    else
+        cudaFree(p);
+}
+
+// RAII bracket that counts a launch and, with profiling on, times it with events on the context's stream.
+struct LaunchScope {
+    fd_ctx* c;
+    int id;
+    cudaEvent_t a = nullptr, b = nullptr;
+    LaunchScope(fd_ctx* c_, int id_) : c(c_), id(id_) {
+        c->launches++;
+        if (!c->profiling) return;
+        auto get = [&]() {
+            cudaEvent_t e;
+            if (!c->pool.empty()) {
+                e = c->pool.back();
+                c->pool.pop_back();
+            } else {
+                cudaEventCreate(&e);
+            }
+            return e;
+        };
+        a = get();
+        b = get();
+        cudaEventRecord(a, c->stream);
+    }
+    ~LaunchScope() {
+        if (!a) return;
+        cudaEventRecord(b, c->stream);
+        c->pending.push_back({id, a, b});
+    }
+};
+
+static int drain_profile(fd_ctx* c) {
+    if (c->pending.empty()) return FD_OK;
+    FD_CUDA(cudaStreamSynchronize(c->stream));
+    for (auto& r : c->pending) {
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, r.a, r.b);
+        c->prof_ms[r.id] += ms;
+        c->prof_n[r.id]++;
+        c->pool.push_back(r.a);
+        c->pool.push_back(r.b);
+    }
+    c->pending.clear();
+    return FD_OK;
+}
+
+template <class T>
+static Coef<T> make_coef(const fd_ctx* c) {
+    // Coefficients are formed in double and rounded once to T (reading G13: constant folding is free).
+    const double dx = c->dx, dx2 = dx * dx;
+    Coef<T> k;
+    k.a1 = T(45.0 / (60.0 * dx));
+    k.a2 = T(-9.0 / (60.0 * dx));
+    k.a3 = T(1.0 / (60.0 * dx));
+    k.b0 = T(-490.0 / (180.0 * dx2));
+    k.b1 = T(270.0 / (180.0 * dx2));
+    k.b2 = T(-27.0 / (180.0 * dx2));
+    k.b3 = T(2.0 / (180.0 * dx2));
+    k.m1 = T(270.0 / (720.0 * dx2));
+    k.m2 = T(-27.0 / (720.0 * dx2));
+    k.m3 = T(2.0 / (720.0 * dx2));
+    k.nu = T(c->nu);
+    k.nu3 = T(c->nu / 3.0);
+    k.cs2 = T(c->cs * c->cs);
+    return k;
+}
+
+// Williamson 2N-RK3 (reading G2); written here and in the oracle independently.
+static const double kAlpha[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
+static const double kBeta[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+
+// ------------------------------------------------------------------------------------------------
+// launch helpers (typed)
+// ------------------------------------------------------------------------------------------------
+template <class T>
+static int launch_halo(fd_ctx* c, T* F, int nfields) {
+    const Geom& g = c->g;
+    {
+        LaunchScope ls(c, FD_K_HALO_X);
+        long long threads = (long long)g.ny * g.nz * nfields;
+        k_halo_x<T><<<(unsigned)((threads + 127) / 128), 128, 0, c->stream>>>(F, g, nfields);
+    }
+    {
+        LaunchScope ls(c, FD_K_HALO_YZ);
+        dim3 grid(2 * R * g.py + 2 * R * g.nz, nfields);
+        k_halo_yz<T><<<grid, 128, 0, c->stream>>>(F, g);
+    }
+    FD_CUDA(cudaGetLastError());
+    return FD_OK;
+}
+
+// One substep of the selected path: F[cur] (valid ghosts) -> F[1-cur] (+ghosts if write_f), w updated.
+template <class T>
+static int launch_substep(fd_ctx* c, const Sub<T>& s) {
+    const Geom& g = c->g;
+    const Coef<T> k = make_coef<T>(c);
+    const T* Fin = (const T*)c->F[c->cur];
+    T* Fout = (T*)c->F[1 - c->cur];
+    T* W = (T*)c->W;
+    T* Div = (T*)c->Div;
+    if (c->variant == FD_VARIANT_TILED) {
+        int rc = tiled_substep<T>(c->tiled, c->path, c->cur, Fin, Fout, W, Div, g, k, s, c->stream,
+                                  [&](int id) { return LaunchScope(c, id); },
+                                  [&](T* f, int nf) { return launch_halo<T>(c, f, nf); });
+        if (rc != FD_OK) return fail(rc, "tiled substep failed: %s", cudaGetErrorString(cudaGetLastError()));
+    } else {
+        dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
+        if (c->path == FD_PATH_55) {
+            LaunchScope ls(c, FD_K_FUSED55);
+            k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
+        } else {
+            {
+                LaunchScope ls(c, FD_K_PASS1);
+                k_direct_main<T, false><<<grid, block, 0, c->stream>>>(Fin, Fout, W, Div, g, k, s);
+            }
+            int rc = launch_halo<T>(c, Div, 1);  // "Compute boundary conditions for (div u)" (Alg. 3)
+            if (rc) return rc;
+            LaunchScope ls(c, FD_K_PASS2);
+            k_direct_pass2<T><<<grid, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+        }
+        FD_CUDA(cudaGetLastError());
+    }
+    if (s.write_f) {
+        int rc = launch_halo<T>(c, Fout, 4);  // ghosts of the new state, ready for the next RHS (reading G12)
+        if (rc) return rc;
+        c->cur = 1 - c->cur;  // "swapped efficiently using pointers"
+    }
+    return FD_OK;
+}
+
+template <class T>
+static int do_rk3(fd_ctx* c, double dt, int nsteps) {
+    for (int n = 0; n < nsteps; ++n)
+        for (int s = 0; s < 3; ++s) {
+            Sub<T> sub;
+            sub.alpha = T(kAlpha[s]);
+            sub.beta = T(kBeta[s]);
+            sub.dt = T(dt);
+            sub.read_w = s != 0;  // alpha^(1) = 0: w is not read
+            sub.write_f = 1;
+            int rc = launch_substep<T>(c, sub);
+            if (rc) return rc;
+        }
+    return FD_OK;
+}
+
+template <class T>
+static int do_pack(fd_ctx* c, const T* const src[4]) {
+    const Geom& g = c->g;
+    T* F = (T*)c->F[c->cur];
+    {
+        LaunchScope ls(c, FD_K_PACK);
+        dim3 grid((g.nx + 127) / 128, g.ny, g.nz * 4);
+        k_pack<T><<<grid, 128, 0, c->stream>>>(src[0], src[1], src[2], src[3], F, g);
+    }
+    FD_CUDA(cudaGetLastError());
+    return launch_halo<T>(c, F, 4);
+}
+
+template <class T>
+static int do_unpack(fd_ctx* c, const T* F, T* const dst[4]) {
+    const Geom& g = c->g;
+    LaunchScope ls(c, FD_K_UNPACK);
+    dim3 grid((g.nx + 127) / 128, g.ny, g.nz * 4);
+    k_unpack<T><<<grid, 128, 0, c->stream>>>(F, dst[0], dst[1], dst[2], dst[3], g);
+    FD_CUDA(cudaGetLastError());
+    return FD_OK;
+}
+
+template <class T>
+static int do_load(fd_ctx* c, const void* const in[4], int where) {
+    const size_t nb = (size_t)c->g.n * sizeof(T);
+    const T* src[4];
+    for (int q = 0; q < 4; ++q) {
+        if (where == FD_HOST) {
+            T* stage = (T*)c->W + (size_t)q * c->g.n;  // w is scratch between steps (alpha_1 = 0)
+            FD_CUDA(cudaMemcpyAsync(stage, in[q], nb, cudaMemcpyHostToDevice, c->stream));
+            src[q] = stage;
+        } else {
+            src[q] = (const T*)in[q];
+        }
+    }
+    int rc = do_pack<T>(c, src);
+    if (rc) return rc;
+    if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
+    return FD_OK;
+}
+
+template <class T>
+static int copy_out(fd_ctx* c, const T* dense_w, void* const out[4]) {
+    // dense_w: four dense arrays in W, to the caller's host arrays.
+    const size_t nb = (size_t)c->g.n * sizeof(T);
+    for (int q = 0; q < 4; ++q)
+        FD_CUDA(cudaMemcpyAsync(out[q], dense_w + (size_t)q * c->g.n, nb, cudaMemcpyDeviceToHost, c->stream));
+    FD_CUDA(cudaStreamSynchronize(c->stream));
+    return FD_OK;
+}
+
+template <class T>
+static int do_store(fd_ctx* c, void* const out[4], int where) {
+    T* dst[4];
+    for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (T*)c->W + (size_t)q * c->g.n : (T*)out[q];
+    int rc = do_unpack<T>(c, (const T*)c->F[c->cur], dst);
+    if (rc) return rc;
+    return where == FD_HOST ? copy_out<T>(c, (const T*)c->W, out) : FD_OK;
+}
+
+template <class T>
+static int do_rhs(fd_ctx* c, void* const out[4], int where) {
+    Sub<T> sub;
+    sub.alpha = T(0);
+    sub.beta = T(0);
+    sub.dt = T(1);
+    sub.read_w = 0;
+    sub.write_f = 0;  // w <- rhs, state untouched
+    int rc = launch_substep<T>(c, sub);
+    if (rc) return rc;
+    const size_t nb = (size_t)c->g.n * sizeof(T);
+    for (int q = 0; q < 4; ++q)
+        FD_CUDA(cudaMemcpyAsync(out[q], (const T*)c->W + (size_t)q * c->g.n, nb,
+                                where == FD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+    if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
+    return FD_OK;
+}
+
+static int resolve_variant(fd_ctx* c) {
+    int want = c->variant_req;
+    bool tiled_ok = tiled_supported(c->g, c->dtype);
+    if (want == FD_VARIANT_AUTO) want = tiled_ok ? FD_VARIANT_TILED : FD_VARIANT_DIRECT;
+    if (want == FD_VARIANT_TILED) {
+        if (!tiled_ok) return fail(FD_EUNSUPPORTED, "tiled variant does not support this grid");
+        int rc = tiled_prepare(c->tiled, c->g, c->dtype, c->F[0], c->F[1], c->Div);
+        if (rc != FD_OK) {
+            if (c->variant_req == FD_VARIANT_AUTO) {
+                want = FD_VARIANT_DIRECT;
+            } else {
+                return fail(rc, "tiled variant setup failed: %s", tiled_error());
+            }
+        }
+    }
+    c->variant = want;
+    return FD_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+#define FD_CHECK_CTX(c) \
+    if (!(c)) return fail(FD_EINVAL, "%s: ctx is NULL", __func__)
+
+extern "C" const char* fd_last_error(void) { return g_err; }
+
+extern "C" int fd_create(fd_ctx** out, int nx, int ny, int nz, double dx, double nu, double cs, int dtype) {
+    if (!out) return fail(FD_EINVAL, "fd_create: out is NULL");
+    *out = nullptr;
+    if (nx < 8 || ny < 8 || nz < 8) return fail(FD_EINVAL, "fd_create: every axis needs n >= 8 (got %d,%d,%d)", nx, ny, nz);
+    if (!(dx > 0) || !std::isfinite(dx)) return fail(FD_EINVAL, "fd_create: dx must be finite and > 0");
+    if (!(nu >= 0) || !std::isfinite(nu)) return fail(FD_EINVAL, "fd_create: nu must be finite and >= 0");
+    if (!(cs >= 0) || !std::isfinite(cs)) return fail(FD_EINVAL, "fd_create: cs must be finite and >= 0");
+    if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_create: bad dtype %d", dtype);
+    if (nx % 4 != 0) return fail(FD_EUNSUPPORTED, "fd_create: nx must be a multiple of 4 (got %d)", nx);
+    if ((long long)nx * ny * nz > (1LL << 33)) return fail(FD_EUNSUPPORTED, "fd_create: grid too large");
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(FD_ECUDA, "fd_create: no CUDA device (%s); libfd6 has no CPU fallback", cudaGetErrorString(e));
+    }
+    fd_ctx* c = new (std::nothrow) fd_ctx();
+    if (!c) return fail(FD_ENOMEM, "fd_create: host allocation failed");
+    c->dtype = dtype;
+    c->esize = dtype == FD_F32 ? 4 : 8;
+    c->dx = dx;
+    c->nu = nu;
+    c->cs = cs;
+    c->alloc = g_alloc;
+    c->release = g_free;
+    c->alloc_user = g_alloc_user;
+    // HBM layout: 32-byte ghost pad in x so interior rows start sector-aligned and 16-byte vector /
+    // TMA accesses are legal; row pitch a multiple of 32 bytes; 3 ghost rows / planes in y and z.
+    Geom& g = c->g;
+    const int e32 = (int)(32 / c->esize);
+    g.nx = nx;
+    g.ny = ny;
+    g.nz = nz;
+    g.gx = e32;
+    g.gy = R;
+    g.gz = R;
+    g.px = ((nx + 2 * g.gx + e32 - 1) / e32) * e32;
+    g.py = ny + 2 * R;
+    g.pz = nz + 2 * R;
+    g.n = (long long)nx * ny * nz;
+    long long fs = (long long)g.px * g.py * g.pz;
+    const long long e256 = (long long)(256 / c->esize);
+    g.fs = ((fs + e256 - 1) / e256) * e256;
+    int rc = FD_OK;
+    for (int b = 0; b < 2 && rc == FD_OK; ++b) {
+        rc = ctx_alloc(c, &c->F[b], (size_t)g.fs * 4 * c->esize);
+        if (rc == FD_OK && cudaMemsetAsync(c->F[b], 0, (size_t)g.fs * 4 * c->esize, c->stream) != cudaSuccess)
+            rc = fail(FD_ECUDA, "fd_create: memset failed: %s", cudaGetErrorString(cudaGetLastError()));
+    }
+    if (rc == FD_OK) rc = ctx_alloc(c, &c->W, (size_t)g.n * 4 * c->esize);
+    if (rc == FD_OK && cudaMemsetAsync(c->W, 0, (size_t)g.n * 4 * c->esize, c->stream) != cudaSuccess)
+        rc = fail(FD_ECUDA, "fd_create: memset failed: %s", cudaGetErrorString(cudaGetLastError()));
+    if (rc == FD_OK) rc = resolve_variant(c);
+    if (rc != FD_OK) {
+        char keep[sizeof(g_err)];
+        strncpy(keep, g_err, sizeof(keep));
+        fd_destroy(c);
+        strncpy(g_err, keep, sizeof(g_err));
+        return rc;
+    }
+    *out = c;
+    return FD_OK;
+}
+
+extern "C" int fd_destroy(fd_ctx* c) {
+    if (!c) return FD_OK;
+    cudaStreamSynchronize(c->stream);
+    for (auto& r : c->pending) {
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    for (auto& ev : c->pool) cudaEventDestroy(ev);
+    tiled_release(c->tiled);
+    ctx_free(c, c->F[0]);
+    ctx_free(c, c->F[1]);
+    ctx_free(c, c->W);
+    ctx_free(c, c->Div);
+    cudaGetLastError();
+    delete c;
+    return FD_OK;
+}
+
+extern "C" int fd_set_path(fd_ctx* c, int path) {
+    FD_CHECK_CTX(c);
+    if (path != FD_PATH_55 && path != FD_PATH_19) return fail(FD_EINVAL, "fd_set_path: bad path %d", path);
+    if (path == FD_PATH_19 && !c->Div) {
+        int rc = ctx_alloc(c, &c->Div, (size_t)c->g.fs * c->esize);
+        if (rc) return rc;
+        FD_CUDA(cudaMemsetAsync(c->Div, 0, (size_t)c->g.fs * c->esize, c->stream));
+        c->path = path;
+        return resolve_variant(c);  // the tiled variant needs a tensor map of the div array
+    }
+    c->path = path;
+    return FD_OK;
+}
+
+extern "C" int fd_set_variant(fd_ctx* c, int variant) {
+    FD_CHECK_CTX(c);
+    if (variant < FD_VARIANT_AUTO || variant > FD_VARIANT_TILED) return fail(FD_EINVAL, "fd_set_variant: bad variant %d", variant);
+    int old = c->variant_req;
+    c->variant_req = variant;
+    int rc = resolve_variant(c);
+    if (rc) c->variant_req = old;
+    return rc;
+}
+
+extern "C" int fd_set_stream(fd_ctx* c, void* s) {
+    FD_CHECK_CTX(c);
+    if ((cudaStream_t)s != c->stream) {
+        int rc = drain_profile(c);
+        if (rc) return rc;
+        FD_CUDA(cudaStreamSynchronize(c->stream));  // keep ordering across a stream change
+    }
+    c->stream = (cudaStream_t)s;
+    return FD_OK;
+}
+
+static int check_ptrs(const char* fn, const void* a, const void* b, const void* c_, const void* d, int where) {
+    if (!a || !b || !c_ || !d) return fail(FD_EINVAL, "%s: NULL field pointer", fn);
+    if (where != FD_HOST && where != FD_DEVICE) return fail(FD_EINVAL, "%s: bad `where` %d", fn, where);
+    return FD_OK;
+}
+
+extern "C" int fd_load(fd_ctx* c, const void* lnrho, const void* ux, const void* uy, const void* uz, int where) {
+    FD_CHECK_CTX(c);
+    int rc = check_ptrs("fd_load", lnrho, ux, uy, uz, where);
+    if (rc) return rc;
+    const void* in[4] = {lnrho, ux, uy, uz};
+    return c->dtype == FD_F32 ? do_load<float>(c, in, where) : do_load<double>(c, in, where);
+}
+
+extern "C" int fd_store(fd_ctx* c, void* lnrho, void* ux, void* uy, void* uz, int where) {
+    FD_CHECK_CTX(c);
+    int rc = check_ptrs("fd_store", lnrho, ux, uy, uz, where);
+    if (rc) return rc;
+    void* out[4] = {lnrho, ux, uy, uz};
+    return c->dtype == FD_F32 ? do_store<float>(c, out, where) : do_store<double>(c, out, where);
+}
+
+extern "C" int fd_rhs(fd_ctx* c, void* r0, void* r1, void* r2, void* r3, int where) {
+    FD_CHECK_CTX(c);
+    int rc = check_ptrs("fd_rhs", r0, r1, r2, r3, where);
+    if (rc) return rc;
+    void* out[4] = {r0, r1, r2, r3};
+    return c->dtype == FD_F32 ? do_rhs<float>(c, out, where) : do_rhs<double>(c, out, where);
+}
+
+extern "C" int fd_rk3_step(fd_ctx* c, double dt, int nsteps) {
+    FD_CHECK_CTX(c);
+    if (nsteps < 0) return fail(FD_EINVAL, "fd_rk3_step: nsteps < 0");
+    if (!std::isfinite(dt)) return fail(FD_EINVAL, "fd_rk3_step: dt is not finite");
+    return c->dtype == FD_F32 ? do_rk3<float>(c, dt, nsteps) : do_rk3<double>(c, dt, nsteps);
+}
+
+extern "C" int fd_sync(fd_ctx* c) {
+    FD_CHECK_CTX(c);
+    FD_CUDA(cudaStreamSynchronize(c->stream));
+    FD_CUDA(cudaGetLastError());
+    return FD_OK;
+}
+
+extern "C" int fd_get_info(const fd_ctx* c, fd_info* o) {
+    FD_CHECK_CTX(c);
+    if (!o) return fail(FD_EINVAL, "fd_get_info: out is NULL");
+    const Geom& g = c->g;
+    o->nx = g.nx;
+    o->ny = g.ny;
+    o->nz = g.nz;
+    o->dtype = c->dtype;
+    o->path = c->path;
+    o->variant = c->variant;
+    o->pitch_x = g.px;
+    o->pitch_y = g.py;
+    o->pitch_z = g.pz;
+    o->ghost_x = g.gx;
+    o->ghost_y = g.gy;
+    o->ghost_z = g.gz;
+    o->field_stride = (size_t)g.fs;
+    o->device_bytes = c->bytes;
+    return FD_OK;
+}
+
+extern "C" unsigned long long fd_kernel_launches(const fd_ctx* c) { return c ? c->launches : 0ULL; }
+
+extern "C" int fd_set_profiling(fd_ctx* c, int on) {
+    FD_CHECK_CTX(c);
+    if (!on) {
+        int rc = drain_profile(c);
+        if (rc) return rc;
+    }
+    c->profiling = on != 0;
+    return FD_OK;
+}
+
+extern "C" int fd_get_profile(fd_ctx* c, int id, double* ms, unsigned long long* n) {
+    FD_CHECK_CTX(c);
+    if (id < 0 || id >= FD_K_COUNT) return fail(FD_EINVAL, "fd_get_profile: bad kernel id %d", id);
+    int rc = drain_profile(c);
+    if (rc) return rc;
+    if (ms) *ms = c->prof_ms[id];
+    if (n) *n = c->prof_n[id];
+    return FD_OK;
+}
+
+extern "C" int fd_reset_profile(fd_ctx* c) {
+    FD_CHECK_CTX(c);
+    int rc = drain_profile(c);
+    if (rc) return rc;
+    for (int i = 0; i < FD_K_COUNT; ++i) {
+        c->prof_ms[i] = 0;
+        c->prof_n[i] = 0;
+    }
+    return FD_OK;
+}
+
+template <class T>
+static int do_poison(fd_ctx* c, bool ghosts) {
+    const T nan = T(NAN);
+    if (ghosts) {
+        long long n = (long long)c->g.px * c->g.py * c->g.pz * 4;
+        for (int b = 0; b < 2; ++b) {
+            c->launches++;
+            k_poison_ghosts<T><<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((T*)c->F[b], c->g, nan);
+        }
+    } else {
+        long long n = c->g.n * 4;
+        c->launches++;
+        k_fill<T><<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>((T*)c->W, n, nan);
+    }
+    FD_CUDA(cudaGetLastError());
+    return FD_OK;
+}
+
+extern "C" int fd_debug_poison_w(fd_ctx* c) {
+    FD_CHECK_CTX(c);
+    return c->dtype == FD_F32 ? do_poison<float>(c, false) : do_poison<double>(c, false);
+}
+
+extern "C" int fd_debug_poison_ghosts(fd_ctx* c) {
+    FD_CHECK_CTX(c);
+    return c->dtype == FD_F32 ? do_poison<float>(c, true) : do_poison<double>(c, true);
+}

@@ -1,0 +1,85 @@
+// fd6_common.cuh — shared device-side definitions of libfd6 (product code; shares nothing with oracle/).
+//
+// Notation follows the paper: F = (ln rho, u_x, u_y, u_z), w = the 2N-RK intermediate
+// arrays, R = stencil radius 3.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace fd6 {
+
+constexpr int R = 3;  // stencil radius, "For both stencils, R = 3"
+
+// Ghost-padded array geometry.  Cell (i,j,k) of a padded field lives at
+//   (i + gx) + px * ((j + gy) + py * (k + gz));  the four fields of one copy are fs elements apart.
+struct Geom {
+    int nx, ny, nz;
+    int px, py, pz;
+    int gx, gy, gz;
+    long long fs;  // padded field stride (elements)
+    long long n;   // nx*ny*nz, the dense (w) field stride
+};
+
+// Stencil coefficients of Eq. 6-8 pre-divided by their denominators, and the physics constants.
+template <class T>
+struct Coef {
+    T a1, a2, a3;      // Eq. 6:  45, -9, 1   over 60 dx
+    T b0, b1, b2, b3;  // Eq. 7: -490, 270, -27, 2 over 180 dx^2
+    T m1, m2, m3;      // Eq. 8:  270, -27, 2 over 720 dx^2
+    T nu, nu3, cs2;    // nu, nu/3, cs^2
+};
+
+// One RK substep (Eq. 10):  w <- alpha w + dt rhs ; F_out <- F + beta w.
+//   read_w == 0  : alpha is 0 and w is NOT read (alpha^(1) = 0; stale/NaN w cannot leak)
+//   write_f == 0 : only w is written (fd_rhs uses alpha = 0, dt = 1 to obtain the plain right-hand side)
+template <class T>
+struct Sub {
+    T alpha, beta, dt;
+    int read_w, write_f;
+};
+
+// Eq. 6 / 7 / 8 around pointer f with element strides s (one axis) or sa, sb (a plane).
+template <class T>
+__device__ __forceinline__ T d1(const T* __restrict__ f, long long s, const Coef<T>& c) {
+    return c.a1 * (f[s] - f[-s]) + c.a2 * (f[2 * s] - f[-2 * s]) + c.a3 * (f[3 * s] - f[-3 * s]);
+}
+template <class T>
+__device__ __forceinline__ T d2(const T* __restrict__ f, long long s, const Coef<T>& c) {
+    return c.b0 * f[0] + c.b1 * (f[s] + f[-s]) + c.b2 * (f[2 * s] + f[-2 * s]) + c.b3 * (f[3 * s] + f[-3 * s]);
+}
+template <class T>
+__device__ __forceinline__ T dmix(const T* __restrict__ f, long long sa, long long sb, const Coef<T>& c) {
+    T q1 = (f[sa + sb] - f[-sa + sb]) + (f[-sa - sb] - f[sa - sb]);
+    T q2 = (f[2 * sa + 2 * sb] - f[-2 * sa + 2 * sb]) + (f[-2 * sa - 2 * sb] - f[2 * sa - 2 * sb]);
+    T q3 = (f[3 * sa + 3 * sb] - f[-3 * sa + 3 * sb]) + (f[-3 * sa - 3 * sb] - f[3 * sa - 3 * sb]);
+    return c.m1 * q1 + c.m2 * q2 + c.m3 * q3;
+}
+
+// Eq. 1-3 assembled from the derivative values at one cell.
+//   u[i]; g[j] = d_j ln rho; G[i][j] = d_j u_i; L[i] = sum_j d_jj u_i; Q[i] = (grad div u)_i (ignored if !withQ).
+// R[0] = -u.g - div u;  R[1+i] = -u.grad u_i - cs^2 g_i + nu (L_i + Q_i/3 + 2 S_ij g_j),
+// S_ij = (G_ij + G_ji)/2 - delta_ij div/3  =>  2 S_ij g_j = sum_j (G_ij + G_ji) g_j - (2/3) div g_i.
+template <class T, bool withQ>
+__device__ __forceinline__ void assemble(const T u[3], const T g[3], const T G[3][3], const T L[3], const T Q[3],
+                                         const Coef<T>& c, T Rout[4]) {
+    const T div = G[0][0] + G[1][1] + G[2][2];
+    Rout[0] = -(u[0] * g[0] + u[1] * g[1] + u[2] * g[2]) - div;
+    const T twothirds_div = T(2.0 / 3.0) * div;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+        T adv = u[0] * G[i][0] + u[1] * G[i][1] + u[2] * G[i][2];
+        T sg = (G[i][0] + G[0][i]) * g[0] + (G[i][1] + G[1][i]) * g[1] + (G[i][2] + G[2][i]) * g[2] - twothirds_div * g[i];
+        T visc = L[i] + sg;
+        T r = c.nu * visc - adv - c.cs2 * g[i];
+        if (withQ) r += c.nu3 * Q[i];
+        Rout[1 + i] = r;
+    }
+}
+
+// Eq. 10 on one value.
+template <class T>
+__device__ __forceinline__ T rk_w(const Sub<T>& s, T rhs, const T* __restrict__ w_ptr) {
+    return s.read_w ? s.alpha * (*w_ptr) + s.dt * rhs : s.dt * rhs;
+}
+
+}  // namespace fd6

@@ -1,0 +1,171 @@
+// fd6_kernels_direct.cuh — layout kernels (pack/unpack, periodic halo fill) and the FD_VARIANT_DIRECT
+// derivative/update kernels: one thread per cell, neighbours straight from the ghost-padded arrays through
+// L1/L2.  Simple and size-agnostic; the tiled TMA kernels in fd6_kernels_tiled.cuh are the fast path.
+#pragma once
+#include "fd6_common.cuh"
+
+namespace fd6 {
+
+// ------------------------------------------------------------------------------------------------
+// a0  pack / unpack: caller's dense arrays <-> interior of the padded arrays.
+// grid (ceil(nx/128), ny, nz) x 4 fields through blockIdx.z = k + nz*q.
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(128) k_pack(const T* __restrict__ d0, const T* __restrict__ d1_, const T* __restrict__ d2_,
+                                              const T* __restrict__ d3, T* __restrict__ F, Geom g) {
+    int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z % g.nz, q = blockIdx.z / g.nz;
+    if (i >= g.nx) return;
+    const T* src = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
+    F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))] =
+        src[i + (long long)g.nx * (j + (long long)g.ny * k)];
+}
+
+template <class T>
+__global__ void __launch_bounds__(128) k_unpack(const T* __restrict__ F, T* __restrict__ d0, T* __restrict__ d1_,
+                                                T* __restrict__ d2_, T* __restrict__ d3, Geom g) {
+    int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z % g.nz, q = blockIdx.z / g.nz;
+    if (i >= g.nx) return;
+    T* dst = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
+    dst[i + (long long)g.nx * (j + (long long)g.ny * k)] =
+        F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 / a7  periodic halo fill, radius 3 (Alg. 2/3 "Compute boundary conditions").
+//   k_halo_x : every interior row (j,k) copies 3 cells to each x ghost.          thread per (row, field)
+//   k_halo_yz: every ghost ROW (j or k outside the domain) is the x-extended copy of the interior row it
+//              wraps to; run after k_halo_x so edge ghosts (two coordinates outside, needed by the Eq. 8
+//              diagonals) come along.  Corner ghosts are filled too (never read).
+// ------------------------------------------------------------------------------------------------
+template <class T>
+__global__ void __launch_bounds__(128) k_halo_x(T* __restrict__ F, Geom g, int nfields) {
+    long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+    long long rows = (long long)g.ny * g.nz;
+    if (t >= rows * nfields) return;
+    int q = (int)(t / rows);
+    long long r = t - q * rows;
+    int j = (int)(r % g.ny), k = (int)(r / g.ny);
+    T* row = F + q * g.fs + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz)) + g.gx;
+#pragma unroll
+    for (int m = 0; m < R; ++m) {
+        row[-1 - m] = row[g.nx - 1 - m];
+        row[g.nx + m] = row[m];
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(128) k_halo_yz(T* __restrict__ F, Geom g) {
+    // blockIdx.x enumerates ghost rows: first the 2R ghost z-planes (py rows each), then for every
+    // interior plane its 2R ghost y-rows.  blockIdx.y = field.
+    int b = blockIdx.x, jj, kk;
+    const int zrows = 2 * R * g.py;
+    if (b < zrows) {
+        int zp = b / g.py;
+        jj = b - zp * g.py;
+        kk = zp < R ? zp + (g.gz - R) : g.gz + g.nz + (zp - R);
+    } else {
+        b -= zrows;
+        int k = b / (2 * R), yr = b - k * (2 * R);
+        kk = k + g.gz;
+        jj = yr < R ? yr + (g.gy - R) : g.gy + g.ny + (yr - R);
+    }
+    int js = jj - g.gy, ks = kk - g.gz;  // wrap to the interior row (n >= 8 > R: one correction suffices)
+    js += js < 0 ? g.ny : 0;
+    js -= js >= g.ny ? g.ny : 0;
+    ks += ks < 0 ? g.nz : 0;
+    ks -= ks >= g.nz ? g.nz : 0;
+    T* base = F + blockIdx.y * g.fs;
+    T* dst = base + (long long)g.px * (jj + (long long)g.py * kk) + (g.gx - R);
+    const T* src = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz)) + (g.gx - R);
+    for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = src[x];
+}
+
+// ------------------------------------------------------------------------------------------------
+// a2-a4 (PATH55 = true) fused 55-point kernel:  27 derivatives, Eq. 1-3, Eq. 10           (Alg. 2)
+// a6    (PATH55 = false) 19-point pass 1: div u to global, partial update without nu/3 grad div (Eq. 14-16)
+// block (64,4,1), grid (ceil(nx/64), ceil(ny/4), nz): one thread per cell.
+// ------------------------------------------------------------------------------------------------
+template <class T, bool PATH55>
+__global__ void __launch_bounds__(256) k_direct_main(const T* __restrict__ Fin, T* __restrict__ Fout, T* __restrict__ W,
+                                                     T* __restrict__ Div, Geom g, Coef<T> c, Sub<T> s) {
+    int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
+    if (i >= g.nx || j >= g.ny) return;
+    const long long sx = 1, sy = g.px, sz = (long long)g.px * g.py;
+    const long long p = (i + g.gx) + sy * (j + g.gy) + sz * (k + g.gz);
+    const long long pw = i + (long long)g.nx * (j + (long long)g.ny * k);
+    const T* l = Fin + p;
+    const T* uu[3] = {Fin + g.fs + p, Fin + 2 * g.fs + p, Fin + 3 * g.fs + p};
+    const long long st[3] = {sx, sy, sz};
+
+    T u[3], gl[3], G[3][3], L[3], Q[3] = {T(0), T(0), T(0)};
+#pragma unroll
+    for (int a = 0; a < 3; ++a) gl[a] = d1(l, st[a], c);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        u[q] = uu[q][0];
+        T dd[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            G[q][a] = d1(uu[q], st[a], c);
+            dd[a] = d2(uu[q], st[a], c);
+        }
+        L[q] = dd[0] + dd[1] + dd[2];
+        if (PATH55) Q[q] = dd[q];  // d_qq u_q is shared between the Laplacian and grad div
+    }
+    if (PATH55) {
+        Q[0] += dmix(uu[1], sx, sy, c) + dmix(uu[2], sx, sz, c);
+        Q[1] += dmix(uu[0], sy, sx, c) + dmix(uu[2], sy, sz, c);
+        Q[2] += dmix(uu[0], sz, sx, c) + dmix(uu[1], sz, sy, c);
+    }
+    T Rv[4];
+    assemble<T, PATH55>(u, gl, G, L, Q, c, Rv);
+    if (!PATH55) Div[p] = G[0][0] + G[1][1] + G[2][2];
+    const T fc[4] = {l[0], u[0], u[1], u[2]};
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        T* wp = W + q * g.n + pw;
+        T wn = rk_w(s, Rv[q], wp);
+        *wp = wn;
+        if (s.write_f) Fout[q * g.fs + p] = fc[q] + s.beta * wn;
+    }
+}
+
+// a8  19-point pass 2:  w_i += dt nu/3 D1_i(div) (Eq. 17);  F_out,i += beta dt nu/3 D1_i(div) (Eq. 18).
+template <class T>
+__global__ void __launch_bounds__(256) k_direct_pass2(const T* __restrict__ Div, T* __restrict__ Fout, T* __restrict__ W,
+                                                      Geom g, Coef<T> c, Sub<T> s) {
+    int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
+    if (i >= g.nx || j >= g.ny) return;
+    const long long sy = g.px, sz = (long long)g.px * g.py;
+    const long long p = (i + g.gx) + sy * (j + g.gy) + sz * (k + g.gz);
+    const long long pw = i + (long long)g.nx * (j + (long long)g.ny * k);
+    const long long st[3] = {1, sy, sz};
+    const T scale = s.dt * c.nu3;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        T add = scale * d1(Div + p, st[a], c);
+        T* wp = W + (1 + a) * g.n + pw;
+        *wp += add;
+        if (s.write_f) Fout[(1 + a) * g.fs + p] += s.beta * add;
+    }
+}
+
+// Test hooks: poison w / all ghost cells with NaN.
+template <class T>
+__global__ void k_fill(T* __restrict__ a, long long n, T v) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n) a[t] = v;
+}
+template <class T>
+__global__ void k_poison_ghosts(T* __restrict__ F, Geom g, T v) {
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long per = (long long)g.px * g.py * g.pz;
+    if (t >= per * 4) return;
+    int q = (int)(t / per);
+    long long r = t - q * per;
+    int x = (int)(r % g.px), y = (int)((r / g.px) % g.py), z = (int)(r / ((long long)g.px * g.py));
+    bool interior = x >= g.gx && x < g.gx + g.nx && y >= g.gy && y < g.gy + g.ny && z >= g.gz && z < g.gz + g.nz;
+    if (!interior) F[q * g.fs + r] = v;
+}
+
+}  // namespace fd6

@@ -1,0 +1,83 @@
+"""Boundary checks that need no GPU: libfd6.so loads, exports every symbol include/fd6.h declares, and
+validates its arguments before touching CUDA.  No compute call is made here."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def fd6():
+    from paper_1707_08900_b200 import build
+    build.build()
+    from paper_1707_08900_b200 import fd6 as mod
+    return mod
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "fd6.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(fd_[a-z0-9_]+)\s*\(", src)) - {"fd_alloc_fn", "fd_free_fn"})
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = declared_functions()
+    for must in ("fd_create", "fd_load", "fd_store", "fd_rhs", "fd_rk3_step", "fd_destroy"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(fd6):
+    for name in declared_functions():
+        assert hasattr(fd6.lib, name), f"libfd6.so does not export {name}"
+    assert sorted(fd6.EXPORTS) == declared_functions()
+
+
+def test_library_does_not_link_torch_or_the_oracle(fd6):
+    import subprocess
+    out = subprocess.run(["ldd", os.path.join(ROOT, "paper_1707_08900_b200", "libfd6.so")], capture_output=True, text=True).stdout
+    assert "torch" not in out and "c10" not in out and "fd_oracle" not in out
+
+
+def test_product_sources_never_reference_the_oracle():
+    pkg = os.path.join(ROOT, "paper_1707_08900_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                text = open(os.path.join(dirpath, f)).read()
+                assert "fd_oracle" not in text and "from oracle" not in text and "import oracle" not in text, f
+
+
+def test_argument_validation_happens_before_any_cuda_call(fd6):
+    h = C.c_void_p()
+    L = fd6.lib
+    assert L.fd_create(None, 32, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 4, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert b"n >= 8" in L.fd_last_error()
+    assert L.fd_create(C.byref(h), 32, 32, 7, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 32, 32, 32, 0.0, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 32, 32, 32, float("nan"), 0.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 32, 32, 32, 0.1, -1.0, 1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 32, 32, 32, 0.1, 0.0, -1.0, fd6.FD_F32) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 32, 32, 32, 0.1, 0.0, 1.0, 7) == fd6.FD_EINVAL
+    assert L.fd_create(C.byref(h), 30, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EUNSUPPORTED
+    assert h.value is None
+    # NULL context
+    assert L.fd_rk3_step(None, 0.1, 1) == fd6.FD_EINVAL
+    assert L.fd_load(None, None, None, None, None, 0) == fd6.FD_EINVAL
+    assert L.fd_set_path(None, 0) == fd6.FD_EINVAL
+    assert L.fd_destroy(None) == fd6.FD_OK
+    assert L.fd_kernel_launches(None) == 0
+
+
+def test_no_cpu_fallback_without_a_device(fd6):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    h = C.c_void_p()
+    assert fd6.lib.fd_create(C.byref(h), 32, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_ECUDA
+    assert b"no CPU fallback" in fd6.lib.fd_last_error()
+    with pytest.raises(fd6.FdError):
+        fd6.Fd(32, 32, 32, 0.1, 0.0, 1.0)

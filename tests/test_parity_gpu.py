@@ -1,0 +1,319 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same seeded
+inputs.  Bars (BASELINE.json north_star): max relative L-inf <= 1e-12 (fp64), <= 2e-5 (fp32)
+after one full RK3 step; each stencil path against the oracle of the SAME path (reading G7); fp32 results
+against the DOUBLE oracle on the same fp32-representable inputs (reading G15)."""
+import math
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 2e-5}
+TWO_PI = 2.0 * math.pi
+
+
+@pytest.fixture(scope="module")
+def mods():
+    from oracle import oracle as O
+    from paper_1707_08900_b200 import fd6, inputs
+    return O, fd6, inputs
+
+
+def relinf(A, B):
+    """reading G14: per field max|A-B| / max|B| (absolute if max|B| == 0), max over fields."""
+    worst = 0.0
+    for a, b in zip(A, B):
+        den = float(np.abs(b).max())
+        err = float(np.abs(a.astype(np.float64) - b).max())
+        worst = max(worst, err / den if den > 0 else err)
+    return worst
+
+
+def variants(fd6):
+    return [fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_TILED]
+
+
+def make_ctx(fd6, shape_xyz, dx, nu, cs, dtype, path, variant):
+    nx, ny, nz = shape_xyz
+    ctx = fd6.Fd(nx, ny, nz, dx, nu, cs, fd6.FD_F32 if dtype == "f32" else fd6.FD_F64)
+    ctx.fd_set_path(path)
+    try:
+        ctx.fd_set_variant(variant)
+    except fd6.FdError as e:
+        if e.code == fd6.FD_EUNSUPPORTED:
+            ctx.fd_destroy()
+            pytest.skip("variant does not support this grid")
+        raise
+    return ctx
+
+
+def smooth_state(rng, shape_xyz, amp, dtype):
+    """A few random low-wavenumber modes per field on a (possibly non-cubic) periodic box."""
+    nx, ny, nz = shape_xyz
+    i = np.arange(nx)[None, None, :] / nx
+    j = np.arange(ny)[None, :, None] / ny
+    k = np.arange(nz)[:, None, None] / nz
+    F = np.zeros((4, nz, ny, nx))
+    for q in range(4):
+        for _ in range(4):
+            kv = rng.integers(-2, 3, 3)
+            F[q] += amp * rng.uniform(0.3, 1.0) * np.cos(TWO_PI * (kv[0] * i + kv[1] * j + kv[2] * k) + rng.uniform(0, TWO_PI))
+    return F.astype(np.float32 if dtype == "f32" else np.float64)
+
+
+# ------------------------------------------------------------------ layout: load / store / halo
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("where", ["host", "device"])
+def test_load_store_round_trip_is_bit_exact(mods, dtype, where):
+    import torch
+    O, fd6, I = mods
+    rng = np.random.default_rng(1)
+    shape = (40, 13, 9)
+    F = rng.standard_normal((4, 9, 13, 40)).astype(np.float32 if dtype == "f32" else np.float64)
+    ctx = make_ctx(fd6, shape, 0.1, 0.01, 1.0, dtype, fd6.FD_PATH_55, fd6.FD_VARIANT_DIRECT)
+    if where == "host":
+        ctx.load_state(F)
+        out = ctx.store_state()
+    else:
+        d = torch.from_numpy(F).cuda()
+        ctx.load_state(d)
+        o = torch.empty_like(d)
+        ctx.store_state(o)
+        ctx.fd_sync()
+        out = o.cpu().numpy()
+    assert np.array_equal(out, F)
+    assert ctx.fd_kernel_launches() > 0
+    ctx.fd_destroy()
+
+
+# ------------------------------------------------------------ config C1: full grid, both paths
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_c1_one_step_and_rhs_full_grid_fp64(mods, path, variant):
+    O, fd6, I = mods
+    cfg = I.CONFIGS["C1"]
+    F = I.make_state(cfg)
+    ctx = make_ctx(fd6, (cfg.n,) * 3, cfg.dx, cfg.nu, cfg.cs, "f64", path, variant)
+    ctx.load_state(F)
+    R = ctx.rhs_state()
+    assert relinf(R, O.rhs(F, cfg.dx, cfg.nu, cfg.cs, path)) <= TOL["f64"]
+    assert np.array_equal(ctx.store_state(), F)  # fd_rhs leaves the state untouched
+    ctx.fd_debug_poison_w()                        # stale w must not matter: alpha^(1) = 0
+    ctx.fd_rk3_step(cfg.dt, 1)
+    got = ctx.store_state()
+    ref = O.rk3_step(F, cfg.dx, cfg.nu, cfg.cs, cfg.dt, 1, path)
+    assert relinf(got, ref) <= TOL["f64"]
+    ctx.fd_destroy()
+
+
+# ------------------------------------------- ragged sizes spanning several tiles plus a tail
+@pytest.mark.parametrize("shape", [(40, 13, 9), (8, 8, 8), (132, 70, 20), (72, 33, 41)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_ragged_grids_three_steps(mods, shape, dtype, path, variant):
+    O, fd6, I = mods
+    rng = np.random.default_rng(shape[0] * 1000 + shape[1] * 10 + path)
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.1, dtype)
+    ctx = make_ctx(fd6, shape, dx, nu, cs, dtype, path, variant)
+    ctx.fd_debug_poison_ghosts()  # every ghost that is read must have been filled by the library
+    ctx.load_state(F)
+    ctx.fd_rk3_step(dt, 1)
+    one = ctx.store_state()
+    ref1 = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 1, path)
+    assert relinf(one, ref1) <= TOL[dtype]
+    ctx.fd_rk3_step(dt, 2)
+    three = ctx.store_state()
+    ref3 = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 3, path)
+    assert relinf(three, ref3) <= 3 * TOL[dtype]
+    ctx.fd_destroy()
+
+
+# --------------------------------------- config C2 (128^3 fp32): one step, full grid, both paths
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_c2_one_step_full_grid_fp32(mods, path, variant):
+    O, fd6, I = mods
+    cfg = I.CONFIGS["C2"]
+    F = I.make_state(cfg)
+    assert F.dtype == np.float32
+    ctx = make_ctx(fd6, (cfg.n,) * 3, cfg.dx, cfg.nu, cfg.cs, "f32", path, variant)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(cfg.dt, 1)
+    got = ctx.store_state()
+    ref = O.rk3_step(F.astype(np.float64), cfg.dx, cfg.nu, cfg.cs, cfg.dt, 1, path)
+    assert relinf(got, ref) <= TOL["f32"]
+    ctx.fd_destroy()
+
+
+# ----------------------------------------------------------- degenerate and invariant cases
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_uniform_state_at_rest_is_a_fixed_point(mods, dtype, path, variant):
+    O, fd6, I = mods
+    shape = (32, 16, 24)
+    F = np.zeros((4, 24, 16, 32), dtype=np.float32 if dtype == "f32" else np.float64)
+    F[0] = 0.731
+    ctx = make_ctx(fd6, shape, 0.1, 5e-3, 1.0, dtype, path, variant)
+    ctx.load_state(F)
+    assert np.all(ctx.rhs_state() == 0.0)
+    ctx.fd_rk3_step(0.01, 2)
+    assert np.array_equal(ctx.store_state(), F)
+    ctx.fd_rk3_step(0.01, 0)  # nsteps = 0 is a no-op
+    assert np.array_equal(ctx.store_state(), F)
+    ctx.fd_destroy()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_periodic_shift_equivariance_is_bitwise(mods, dtype, path, variant):
+    """step(roll(F)) == roll(step(F)) bit for bit: no cell's arithmetic may depend on its position in a tile."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(5)
+    shape = (64, 40, 24)
+    F = smooth_state(rng, shape, 0.1, dtype)
+    sh = (5, 17, 30)
+    outs = []
+    for G in (F, np.roll(F, sh, (1, 2, 3))):
+        ctx = make_ctx(fd6, shape, 0.15, 0.01, 1.0, dtype, path, variant)
+        ctx.load_state(np.ascontiguousarray(G))
+        ctx.fd_rk3_step(0.01, 1)
+        outs.append(ctx.store_state())
+        ctx.fd_destroy()
+    assert np.array_equal(np.roll(outs[0], sh, (1, 2, 3)), outs[1])
+
+
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("variant", [1, 2])
+def test_shear_mode_decay_closed_form_on_gpu(mods, path, variant):
+    """P6 on the GPU: the discrete twin of the paper's Eq. 22 test."""
+    O, fd6, I = mods
+    n, k, u0, nu, nsteps = 32, 5, 1e-2, 5e-3, 10
+    dx = TWO_PI / n
+    dt = 0.1 * dx
+    X = (np.arange(n) * dx)[None, None, :] * np.ones((n, n, 1))
+    F = np.zeros((4, n, n, n))
+    F[2] = u0 * np.sin(k * X)
+    a = k * dx
+    s2 = (490 - 540 * np.cos(a) + 54 * np.cos(2 * a) - 4 * np.cos(3 * a)) / 180
+    z = -nu * dt * s2 / dx ** 2
+    G = 1 + z + z * z / 2 + z ** 3 / 6
+    ctx = make_ctx(fd6, (n,) * 3, dx, nu, 1.0, "f64", path, variant)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(dt, nsteps)
+    out = ctx.store_state()
+    np.testing.assert_allclose(out[2], G ** nsteps * u0 * np.sin(k * X), atol=1e-13 * u0)
+    assert max(np.abs(out[q]).max() for q in (0, 1, 3)) < 1e-15
+    ctx.fd_destroy()
+
+
+# ------------------------------- big grids: windowed oracle on sampled blocks
+def _sample_origins(n, size, rng, extra):
+    pts = [(0, 0, 0), (n - size // 2, n - size // 2, n - size // 2), (n - 7, 3, n // 2)] + list(extra)
+    while len(pts) < 8:
+        pts.append(tuple(int(v) for v in rng.integers(0, n, 3)))
+    return pts
+
+
+def _windowed_check(mods, cfg_name, path, variant, n_override=None, inner=16, nblocks=8):
+    import torch
+    O, fd6, I = mods
+    cfg = I.CONFIGS[cfg_name]
+    n = n_override or cfg.n
+    dx = TWO_PI / n
+    dt = 0.1 * dx / cfg.cs
+    F = I.make_state(cfg, device="cuda", n_override=n_override)
+    ctx = make_ctx(fd6, (n,) * 3, dx, cfg.nu, cfg.cs, cfg.dtype, path, variant)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(dt, 1)
+    out = torch.empty_like(F)
+    ctx.store_state(out)
+    ctx.fd_sync()
+    m = O.window_margin(path)
+    size = inner + 2 * m
+    rng = np.random.default_rng(cfg.seed)
+    # blocks at the periodic seam, at the origin, across tile boundaries (multiples of 64/16) and random ones
+    extra = [(64 - m - 3, 16 - m - 2, n // 2 - m), (n // 2 - m - 1, n - m - 5, 5)]
+    worst = 0.0
+    for origin in _sample_origins(n, size, rng, extra)[:nblocks]:
+        sub = I.gather_block(F, origin, size).astype(np.float64)
+        ref, mm = O.rk3_step_window(sub, dx, cfg.nu, cfg.cs, dt, 1, path)
+        got = I.gather_block(out, tuple(o + m for o in origin), inner)
+        worst = max(worst, relinf(got, ref))
+    ctx.fd_destroy()
+    del F, out
+    torch.cuda.empty_cache()
+    return worst
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_c3_256_fp64_sampled_blocks(mods, path):
+    assert _windowed_check(mods, "C3", path, 0) <= TOL["f64"]
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_c4_512_fp32_sampled_blocks_in_the_bench_configuration(mods, path):
+    """Full headline size, default (AUTO) variant = the launch configuration bench.py times."""
+    assert _windowed_check(mods, "C4", path, 0) <= TOL["f32"]
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_c5_1024_fp32_sampled_blocks(mods, path):
+    import torch
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~80 GB of free device memory")
+    assert _windowed_check(mods, "C5", path, 0, nblocks=6) <= TOL["f32"]
+
+
+def test_c3_256_fp64_full_grid_55(mods):
+    O, fd6, I = mods
+    cfg = I.CONFIGS["C3"]
+    F = I.make_state(cfg, device="cpu").numpy()
+    ctx = make_ctx(fd6, (cfg.n,) * 3, cfg.dx, cfg.nu, cfg.cs, "f64", 0, 0)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(cfg.dt, 1)
+    got = ctx.store_state()
+    ref = O.rk3_step(F, cfg.dx, cfg.nu, cfg.cs, cfg.dt, 1, 0)
+    assert relinf(got, ref) <= TOL["f64"]
+    ctx.fd_destroy()
+
+
+# ------------------------------------------------------------------------ error behaviour
+def test_error_codes_on_a_live_context(mods):
+    O, fd6, I = mods
+    ctx = fd6.Fd(32, 32, 32, 0.1, 0.01, 1.0, fd6.FD_F32)
+    L = fd6.lib
+    assert L.fd_rk3_step(ctx._h, 0.1, -1) == fd6.FD_EINVAL
+    assert L.fd_rk3_step(ctx._h, float("inf"), 1) == fd6.FD_EINVAL
+    assert L.fd_set_path(ctx._h, 5) == fd6.FD_EINVAL
+    assert L.fd_set_variant(ctx._h, 9) == fd6.FD_EINVAL
+    assert L.fd_load(ctx._h, None, None, None, None, fd6.FD_HOST) == fd6.FD_EINVAL
+    a = np.zeros(32 ** 3, dtype=np.float32)
+    p = a.ctypes.data
+    assert L.fd_load(ctx._h, p, p, p, p, 3) == fd6.FD_EINVAL
+    assert L.fd_get_profile(ctx._h, 99, None, None) == fd6.FD_EINVAL
+    info = ctx.fd_get_info()
+    assert (info.nx, info.ny, info.nz) == (32, 32, 32) and info.ghost_y == 3 and info.pitch_x >= 32 + 6
+    assert info.device_bytes >= 12 * 32 ** 3 * 4
+    ctx.fd_destroy()
+
+
+def test_profile_counters_count_the_launches(mods):
+    O, fd6, I = mods
+    ctx = fd6.Fd(64, 64, 64, 0.1, 0.01, 1.0, fd6.FD_F32)
+    ctx.load_state(np.zeros((4, 64, 64, 64), dtype=np.float32))
+    ctx.fd_set_profiling(True)
+    ctx.fd_reset_profile()
+    before = ctx.fd_kernel_launches()
+    ctx.fd_rk3_step(0.01, 2)
+    ms, n = ctx.fd_get_profile(fd6.FD_K_FUSED55)
+    assert n == 6 and ms > 0
+    total = sum(ctx.fd_get_profile(k)[1] for k in range(fd6.FD_K_COUNT))
+    assert total == ctx.fd_kernel_launches() - before
+    ctx.fd_destroy()
