@@ -1,0 +1,344 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the RK3 hot path on B200 (BASELINE.json metric), one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4] [--path 55|19] [--impl ours|reference]
+
+A "step" is one full RK3 step (3 substeps: halo fill + fused 55-point kernel, or the 19-point kernel pair) of
+the whole grid.  Workload at N = 1: config C4 of BASELINE.json (512^3 fp32, seeded band-limited fields,
+|k| <= 32, rms Mach 0.3, nu = 1e-3), the configuration the metric is quoted on; the 2.1 GB state and the
+8.6 GB each substep streams are far larger than the 126 MB L2, so no L2 flush is needed between steps.
+N > 1: independent replicas (the north_star path is single-GPU; no collective is
+invented), value = cells of all ranks x K / max-over-ranks device time.
+
+value        device-resident: K steps in one fd_rk3_step(dt, K) call, CUDA events on the launching stream.
+e2e          the same job through the C ABI with HOST (pinned) buffers: fd_load(host) + fd_rk3_step(dt, K) +
+             fd_store(host), copies inside the timed region; bytes per step = job bytes / K.  The variant
+             with a load and a store around EVERY step is reported as e2e.every_step_io.
+roofline     fused 55-point kernel: algorithmic bytes (16 words/cell/substep) / mean launch
+             duration from the library's per-launch CUDA events (fd_set_profiling) over the timed region.
+cpu_baseline the CPU oracle as it stands, timed on the host cores on a bounded sample (rank 0, N = 1).
+--impl reference   times the oracle only (there is no reference implementation; the oracle is the arm).
+"""
+import argparse
+import json
+import math
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mcell-updates/s per full RK3 step"
+UNIT = "Mcell-updates/s"
+WORDS_PER_CELL_SUBSTEP = {"55": 16, "19": 30}  # SURVEY.md 8(d), DESIGN.md "Kernels"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at C4, from the committed
+# `ncu --set full` capture (profiles/); None until that capture exists for the kernel bench.py times.
+NCU_TRAFFIC_BYTES = {}
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.01):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        names = {
+            "hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+            "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+            "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+            "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4),
+            "hw_power_brake": getattr(nv, "nvmlClocksEventReasonHwPowerBrakeSlowdown", 0x80),
+        }
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, bit in names.items():
+                    if mask & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def load_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy bandwidth)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): the ONLY place bench.py touches oracle/.
+# --------------------------------------------------------------------------------------------------
+def oracle_sample(cfg, path_name, budget_s, n_sample=None):
+    """Time the oracle, as it stands, in the config's dtype on a bounded sample of the workload: the config's
+    own recipe on an n_sample^3 periodic grid (same spectrum, dx, dt, nu), 1 step + as many more as fit."""
+    import numpy as np
+    from oracle import oracle as O
+    from paper_1707_08900_b200 import inputs
+
+    n = n_sample or min(cfg.n, 128)
+    F = inputs.make_state(cfg, device="cpu", n_override=n)
+    F = F if isinstance(F, np.ndarray) else F.numpy()
+    dt_np = cfg.np_dtype
+    path = O.PATH_55 if path_name == "55" else O.PATH_19
+    dx = 2 * math.pi / n
+    dt = 0.1 * dx / cfg.cs
+    O.rk3_step(F[:, :16, :16, :16], dx, cfg.nu, cfg.cs, dt, 1, path, dtype=dt_np)  # builds/loads the library
+    t0 = time.perf_counter()
+    G = O.rk3_step(F, dx, cfg.nu, cfg.cs, dt, 1, path, dtype=dt_np)
+    t1 = time.perf_counter() - t0
+    more = int(max(0, min(50, math.floor((budget_s - t1) / max(t1, 1e-3)))))
+    total_steps, total_t = 1, t1
+    if more > 0:
+        t0 = time.perf_counter()
+        O.rk3_step(G, dx, cfg.nu, cfg.cs, dt, more, path, dtype=dt_np)
+        total_t += time.perf_counter() - t0
+        total_steps += more
+    value = n ** 3 * total_steps / total_t / 1e6
+    return {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle",
+            "sample": f"{cfg.name} recipe on a {n}^3 periodic grid, {cfg.dtype}, {path_name}-point path, "
+                      f"{total_steps} full RK3 steps in {total_t:.1f} s (oracle/fd_oracle.cpp, OpenMP over k-planes)"}, total_t, total_steps, n
+
+
+def run_reference(args, cfg):
+    rank = _env_int("RANK", 0)
+    if rank != 0:
+        return 0
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    # each "step" of this arm = one oracle RK3 step on a bounded sample, sized so the whole run ends in minutes
+    import numpy as np
+    from oracle import oracle as O
+    from paper_1707_08900_b200 import inputs
+    n = 128
+    F = inputs.make_state(cfg, device="cpu", n_override=n)
+    F = F if isinstance(F, np.ndarray) else F.numpy()
+    path = O.PATH_55 if args.path == "55" else O.PATH_19
+    dx = 2 * math.pi / n
+    dt = 0.1 * dx / cfg.cs
+    for _ in range(min(warm, 3)):
+        O.rk3_step(F, dx, cfg.nu, cfg.cs, dt, 1, path, dtype=cfg.np_dtype)
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(steps):
+        F = O.rk3_step(F, dx, cfg.nu, cfg.cs, dt, 1, path, dtype=cfg.np_dtype)
+        done += 1
+        if time.perf_counter() - t0 > 150.0:
+            break
+    el = time.perf_counter() - t0
+    value = n ** 3 * done / el / 1e6
+    sample = (f"{cfg.name} recipe on a {n}^3 periodic grid, {cfg.dtype}, {args.path}-point path, one oracle RK3 step "
+              f"per bench step ({done} timed)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+            "warmup": min(warm, 3), "ms_per_step": el / done * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {cfg.n}^3 periodic {cfg.dtype}, sampled at {n}^3 for the CPU oracle",
+                       "path": args.path},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# --------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", default="C4")
+    ap.add_argument("--path", default="55", choices=["55", "19"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 direct, 2 tiled")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-budget", type=float, default=15.0)
+    args = ap.parse_args()
+
+    from paper_1707_08900_b200 import inputs
+    cfg = inputs.CONFIGS[args.config]
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1707_08900_b200 import fd6  # raises if libfd6.so is missing: no CPU fallback
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (the product path has no CPU fallback)"
+    rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    K, W = max(1, args.steps), max(3, args.warmup)
+    n, N = cfg.n, cfg.n ** 3
+    esize = 4 if cfg.dtype == "f32" else 8
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # seeded synthetic state, generated on the device (harness only) then handed to fd_load
+    F0 = inputs.make_state(cfg, device="cuda")
+    if not isinstance(F0, torch.Tensor):
+        F0 = torch.from_numpy(F0).cuda()
+    ctx = fd6.Fd(n, n, n, cfg.dx, cfg.nu, cfg.cs, fd6.FD_F32 if cfg.dtype == "f32" else fd6.FD_F64)
+    ctx.fd_set_path(fd6.FD_PATH_55 if args.path == "55" else fd6.FD_PATH_19)
+    if args.variant:
+        ctx.fd_set_variant(args.variant)
+    info = ctx.fd_get_info()
+    ctx.load_state(F0)
+    ctx.fd_rk3_step(cfg.dt, W)  # warm-up
+    ctx.load_state(F0)          # timed steps start from the config's state
+    ctx.fd_set_profiling(True)
+    ctx.fd_reset_profile()
+    stream = torch.cuda.current_stream()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    launches0 = ctx.fd_kernel_launches()
+    with ClockSampler(local) as clk:
+        e0.record(stream)
+        ctx.fd_rk3_step(cfg.dt, K)
+        e1.record(stream)
+        barrier()
+    launches = ctx.fd_kernel_launches() - launches0
+    ms = e0.elapsed_time(e1)
+    prof = {fd6.KERNEL_NAMES[k]: ctx.fd_get_profile(k) for k in range(fd6.FD_K_COUNT)}
+    ctx.fd_set_profiling(False)
+    chk = torch.empty_like(F0)
+    ctx.store_state(chk)
+    ctx.fd_sync()
+    finite = bool(torch.isfinite(chk).all().item())
+    del chk
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    value = world * N * K / (ms_max * 1e-3) / 1e6
+
+    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
+    host_in = torch.empty(F0.shape, dtype=F0.dtype, pin_memory=True)
+    host_in.copy_(F0)
+    host_out = torch.empty(F0.shape, dtype=F0.dtype, pin_memory=True)
+    state_bytes = 4 * N * esize
+
+    def e2e_job(nsteps):
+        ctx.load_state(host_in)       # fd_load(FD_HOST): H2D + pack + halo fill
+        ctx.fd_rk3_step(cfg.dt, nsteps)
+        ctx.store_state(host_out)     # fd_store(FD_HOST): unpack + D2H, synchronises
+
+    e2e_job(1)
+    barrier()
+    e0.record(stream)
+    e2e_job(K)
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item())
+    e2e_value = world * N * K / (e2e_ms * 1e-3) / 1e6
+    reps = 3
+    barrier()
+    e0.record(stream)
+    for _ in range(reps):
+        e2e_job(1)
+    e1.record(stream)
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_each = world * N * reps / (float(t.item()) * 1e-3) / 1e6
+    finite = finite and bool(torch.isfinite(host_out).all().item())
+
+    # ---- roofline of the dominant kernel
+    peak, peak_src = load_peak()
+    dom = "fused55" if args.path == "55" else "pass1_19"
+    words = 16 if args.path == "55" else 17
+    dom_ms, dom_n = prof[dom]
+    alg_bytes = words * esize * N
+    achieved = alg_bytes / (dom_ms / dom_n * 1e-3) / 1e9 if dom_n else None
+    kern_share = {k: round(v[0] / ms, 4) for k, v in prof.items() if v[1]}
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": (achieved / peak if achieved else None), "traffic": NCU_TRAFFIC_BYTES.get((args.config, dom)),
+                "algorithmic_bytes_per_launch": alg_bytes, "avg_launch_ms": (dom_ms / dom_n if dom_n else None),
+                "peak_source": peak_src, "kernel_share_of_step": kern_share,
+                "step_frac": WORDS_PER_CELL_SUBSTEP[args.path] * esize * 3 * N * K / (ms_max * 1e-3) / 1e9 / peak}
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu_baseline = oracle_sample(cfg, args.path, args.cpu_budget)[0]
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_max / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": cfg.dtype, "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {n}^3 periodic {cfg.dtype}, band-limited |k|<={cfg.kmax} rms Mach {cfg.amp}, "
+                                   f"nu={cfg.nu}, dt=0.1 dx/cs", "path": f"{args.path}-point",
+                       "variant": {1: "direct", 2: "tiled"}.get(info.variant, str(info.variant)),
+                       "l2": "inputs larger than L2 (2.1 GB state, 8.6 GB streamed per substep); no flush needed",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite},
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
+                    "d2h_bytes_per_step": state_bytes / K,
+                    "job": f"fd_load(host pinned) + fd_rk3_step(dt,{K}) + fd_store(host pinned)", "ms": e2e_ms,
+                    "every_step_io": {"value": e2e_each, "h2d_bytes_per_step": state_bytes,
+                                      "d2h_bytes_per_step": state_bytes}},
+            "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline,
+        }
+        if cpu_baseline is not None:
+            line["cpu_baseline"] = cpu_baseline
+        print(json.dumps(line), flush=True)
+    ctx.fd_destroy()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0 if finite else 1
+
+
+if __name__ == "__main__":
+    sys.exit(main())
