@@ -203,28 +203,26 @@ static int launch_substep(fd_ctx* c, const Sub<T>& s) {
     T* Fout = (T*)c->F[1 - c->cur];
     T* W = (T*)c->W;
     T* Div = (T*)c->Div;
-    if (c->variant == FD_VARIANT_TILED) {
-        int rc = tiled_substep<T>(c->tiled, c->path, c->cur, Fin, Fout, W, Div, g, k, s, c->stream,
-                                  [&](int id) { return LaunchScope(c, id); },
-                                  [&](T* f, int nf) { return launch_halo<T>(c, f, nf); });
-        if (rc != FD_OK) return fail(rc, "tiled substep failed: %s", cudaGetErrorString(cudaGetLastError()));
-    } else {
-        dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
-        if (c->path == FD_PATH_55) {
-            LaunchScope ls(c, FD_K_FUSED55);
+    const bool p55 = c->path == FD_PATH_55;
+    dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
+    {
+        LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
+        if (c->variant == FD_VARIANT_TILED) {
+            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, c->dx, c->nu, c->cs, s, c->stream))
+                return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        } else if (p55) {
             k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
         } else {
-            {
-                LaunchScope ls(c, FD_K_PASS1);
-                k_direct_main<T, false><<<grid, block, 0, c->stream>>>(Fin, Fout, W, Div, g, k, s);
-            }
-            int rc = launch_halo<T>(c, Div, 1);  // "Compute boundary conditions for (div u)" (Alg. 3)
-            if (rc) return rc;
-            LaunchScope ls(c, FD_K_PASS2);
-            k_direct_pass2<T><<<grid, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+            k_direct_main<T, false><<<grid, block, 0, c->stream>>>(Fin, Fout, W, Div, g, k, s);
         }
-        FD_CUDA(cudaGetLastError());
     }
+    if (!p55) {
+        int rc = launch_halo<T>(c, Div, 1);  // "Compute boundary conditions for (div u)" (Alg. 3)
+        if (rc) return rc;
+        LaunchScope ls(c, FD_K_PASS2);
+        k_direct_pass2<T><<<grid, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+    }
+    FD_CUDA(cudaGetLastError());
     if (s.write_f) {
         int rc = launch_halo<T>(c, Fout, 4);  // ghosts of the new state, ready for the next RHS (reading G12)
         if (rc) return rc;
@@ -241,7 +239,8 @@ static int do_rk3(fd_ctx* c, double dt, int nsteps) {
             sub.alpha = T(kAlpha[s]);
             sub.beta = T(kBeta[s]);
             sub.dt = T(dt);
-            sub.read_w = s != 0;  // alpha^(1) = 0: w is not read
+            sub.read_w = s != 0;   // alpha^(1) = 0: w is not read
+            sub.write_w = s != 2;  // ... so the w of the last substep is never read either: not written
             sub.write_f = 1;
             int rc = launch_substep<T>(c, sub);
             if (rc) return rc;
@@ -317,6 +316,7 @@ static int do_rhs(fd_ctx* c, void* const out[4], int where) {
     sub.beta = T(0);
     sub.dt = T(1);
     sub.read_w = 0;
+    sub.write_w = 1;
     sub.write_f = 0;  // w <- rhs, state untouched
     int rc = launch_substep<T>(c, sub);
     if (rc) return rc;
@@ -339,7 +339,7 @@ static int resolve_variant(fd_ctx* c) {
             if (c->variant_req == FD_VARIANT_AUTO) {
                 want = FD_VARIANT_DIRECT;
             } else {
-                return fail(rc, "tiled variant setup failed: %s", tiled_error());
+                return fail(rc, "tiled variant setup failed: %s", tiled_error_of(c->tiled));
             }
         }
     }

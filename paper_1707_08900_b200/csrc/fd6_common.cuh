@@ -32,10 +32,11 @@ struct Coef {
 // One RK substep (Eq. 10):  w <- alpha w + dt rhs ; F_out <- F + beta w.
 //   read_w == 0  : alpha is 0 and w is NOT read (alpha^(1) = 0; stale/NaN w cannot leak)
 //   write_f == 0 : only w is written (fd_rhs uses alpha = 0, dt = 1 to obtain the plain right-hand side)
+//   write_w == 0 : w is not written (last substep of a step: the next substep has alpha = 0 and never reads it)
 template <class T>
 struct Sub {
     T alpha, beta, dt;
-    int read_w, write_f;
+    int read_w, write_f, write_w;
 };
 
 // Eq. 6 / 7 / 8 around pointer f with element strides s (one axis) or sa, sb (a plane).

@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(256) k_direct_main(const T* __restrict__ Fin, 
     for (int q = 0; q < 4; ++q) {
         T* wp = W + q * g.n + pw;
         T wn = rk_w(s, Rv[q], wp);
-        *wp = wn;
+        if (s.write_w) *wp = wn;
         if (s.write_f) Fout[q * g.fs + p] = fc[q] + s.beta * wn;
     }
 }
@@ -145,7 +145,7 @@ __global__ void __launch_bounds__(256) k_direct_pass2(const T* __restrict__ Div,
     for (int a = 0; a < 3; ++a) {
         T add = scale * d1(Div + p, st[a], c);
         T* wp = W + (1 + a) * g.n + pw;
-        *wp += add;
+        if (s.write_w) *wp += add;
         if (s.write_f) Fout[(1 + a) * g.fs + p] += s.beta * add;
     }
 }
