@@ -195,7 +195,7 @@ def main():
     ap.add_argument("--config", default="C4")
     ap.add_argument("--path", default="55", choices=["55", "19"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 direct, 2 tiled")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 direct, 2 tiled, 3 paired")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     args = ap.parse_args()

@@ -43,12 +43,15 @@ enum { FD_PATH_55 = 0, FD_PATH_19 = 1 };  /* stencil path */
 enum { FD_HOST = 0, FD_DEVICE = 1 };      /* where caller pointers live */
 enum { FD_OK = 0, FD_EINVAL = 1, FD_ENOMEM = 2, FD_ECUDA = 3, FD_EUNSUPPORTED = 4 };
 
-/* Kernel implementations of the derivative/update step (fd_set_variant).  Both compute the same path;
- * FD_VARIANT_AUTO picks the fastest one that supports the grid. */
+/* Kernel implementations of the derivative/update step (fd_set_variant).  All compute the same path;
+ * FD_VARIANT_AUTO picks the fastest one that supports the grid (PAIRED for fp32 with an even nz, else TILED).
+ * The device layout is private to the library: PAIRED stores cells (i,j,k) and (i,j,k+nz/2) side by side so
+ * that one packed fp32x2 instruction works on both; switching variants converts a loaded state in place. */
 enum {
     FD_VARIANT_AUTO = 0,
-    FD_VARIANT_DIRECT = 1, /* one thread per cell, neighbours through L1/L2 (simple, any supported size)      */
-    FD_VARIANT_TILED = 2   /* TMA-staged xy tiles in shared memory, register sliding window along z            */
+    FD_VARIANT_DIRECT = 1, /* one thread per cell (or pair), neighbours through L1/L2 (simple, any layout)    */
+    FD_VARIANT_TILED = 2,  /* TMA-staged xy tiles in shared memory, register sliding window along z            */
+    FD_VARIANT_PAIRED = 3  /* TILED on the paired fp32 layout with packed FFMA2 arithmetic (fp32, nz even)     */
 };
 
 /* Kernel ids for fd_get_profile. */
@@ -106,7 +109,8 @@ const char* fd_last_error(void);
 /* Introspection (read-only). */
 typedef struct fd_info {
     int nx, ny, nz, dtype, path, variant; /* variant: the one AUTO resolved to            */
-    int pitch_x, pitch_y, pitch_z;        /* padded array extents in elements             */
+    int pitch_x, pitch_y, pitch_z;        /* padded array extents in values (a value = one cell, or a pair of
+                                             cells in the paired layout, where pitch_z covers nz/2 planes)       */
     int ghost_x, ghost_y, ghost_z;        /* offset of cell (0,0,0) inside a padded array */
     size_t field_stride;                  /* elements between consecutive padded fields   */
     size_t device_bytes;                  /* device memory owned by the context           */

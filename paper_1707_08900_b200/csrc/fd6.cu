@@ -59,10 +59,14 @@ struct ProfRec {
 };
 
 struct fd_ctx {
-    Geom g{};
+    Geom g{};  // geometry in VALUES: cells, or V2 pairs of cells when `paired` (then g.nz = nz / 2)
+    int nx = 0, ny = 0, nz = 0;  // the caller's grid
+    bool paired = false;         // fp32 paired layout: value (i,j,k) = cells (i,j,k) and (i,j,k+nz/2)
+    bool loaded = false;         // a state other than the all-zero one is resident
     int dtype = FD_F32, path = FD_PATH_55, variant_req = FD_VARIANT_AUTO, variant = FD_VARIANT_DIRECT;
     double dx = 0, nu = 0, cs = 0;
-    size_t esize = 4;
+    size_t esize = 4;            // bytes per value
+    size_t f_bytes = 0, div_bytes = 0;  // allocation sizes (cover both layouts)
     cudaStream_t stream = nullptr;
     void* F[2] = {nullptr, nullptr};  // two ghost-padded copies of the four fields (read / write)
     void* W = nullptr;                // four dense w arrays
@@ -149,30 +153,91 @@ static int drain_profile(fd_ctx* c) {
     return FD_OK;
 }
 
+// One RK substep as the host sees it (Eq. 10); see Sub<T> for the flags.
+struct SubD {
+    double alpha, beta, dt;
+    int read_w, write_f, write_w;
+};
+
 template <class T>
 static Coef<T> make_coef(const fd_ctx* c) {
-    // Coefficients are formed in double and rounded once to T (reading G13: constant folding is free).
+    // Coefficients are formed in double and rounded once to the scalar type (reading G13: constant folding is free).
+    typedef typename Scalar<T>::type S;
     const double dx = c->dx, dx2 = dx * dx;
     Coef<T> k;
-    k.a1 = T(45.0 / (60.0 * dx));
-    k.a2 = T(-9.0 / (60.0 * dx));
-    k.a3 = T(1.0 / (60.0 * dx));
-    k.b0 = T(-490.0 / (180.0 * dx2));
-    k.b1 = T(270.0 / (180.0 * dx2));
-    k.b2 = T(-27.0 / (180.0 * dx2));
-    k.b3 = T(2.0 / (180.0 * dx2));
-    k.m1 = T(270.0 / (720.0 * dx2));
-    k.m2 = T(-27.0 / (720.0 * dx2));
-    k.m3 = T(2.0 / (720.0 * dx2));
-    k.nu = T(c->nu);
-    k.nu3 = T(c->nu / 3.0);
-    k.cs2 = T(c->cs * c->cs);
+    k.a1 = T(S(45.0 / (60.0 * dx)));
+    k.a2 = T(S(-9.0 / (60.0 * dx)));
+    k.a3 = T(S(1.0 / (60.0 * dx)));
+    k.b0 = T(S(-490.0 / (180.0 * dx2)));
+    k.b1 = T(S(270.0 / (180.0 * dx2)));
+    k.b2 = T(S(-27.0 / (180.0 * dx2)));
+    k.b3 = T(S(2.0 / (180.0 * dx2)));
+    k.m1 = T(S(270.0 / (720.0 * dx2)));
+    k.m2 = T(S(-27.0 / (720.0 * dx2)));
+    k.m3 = T(S(2.0 / (720.0 * dx2)));
+    k.nu = T(S(c->nu));
+    k.nu3 = T(S(c->nu / 3.0));
+    k.cs2 = T(S(c->cs * c->cs));
     return k;
+}
+
+template <class T>
+static Sub<T> make_sub(const SubD& d) {
+    typedef typename Scalar<T>::type S;
+    Sub<T> s;
+    s.alpha = T(S(d.alpha));
+    s.beta = T(S(d.beta));
+    s.dt = T(S(d.dt));
+    s.read_w = d.read_w;
+    s.write_f = d.write_f;
+    s.write_w = d.write_w;
+    return s;
 }
 
 // Williamson 2N-RK3 (reading G2); written here and in the oracle independently.
 static const double kAlpha[3] = {0.0, -5.0 / 9.0, -153.0 / 128.0};
 static const double kBeta[3] = {1.0 / 3.0, 15.0 / 16.0, 8.0 / 15.0};
+
+// Run `expr` with T = the value type of the context (float, double, or V2 in the paired layout).
+#define FD_DISPATCH(c, expr)                   \
+    ((c)->dtype == FD_F64 ? [&]() {            \
+        typedef double T;                      \
+        return (expr);                         \
+    }()                                        \
+     : (c)->paired ? [&]() {                   \
+           typedef V2 T;                       \
+           return (expr);                      \
+       }()                                     \
+                   : [&]() {                   \
+                         typedef float T;      \
+                         return (expr);        \
+                     }())
+
+// ------------------------------------------------------------------------------------------------
+// geometry
+// ------------------------------------------------------------------------------------------------
+// HBM layout: 32-byte ghost pad in x so interior rows start sector-aligned and 16-byte vector /
+// TMA accesses are legal; row pitch a multiple of 32 bytes; 3 ghost rows / planes in y and z.
+static Geom make_geom(int nx, int ny, int nz, size_t esize, bool paired) {
+    Geom g;
+    const int e32 = (int)(32 / esize);
+    g.nx = nx;
+    g.ny = ny;
+    g.nz = paired ? nz / 2 : nz;
+    g.gx = e32;
+    g.gy = R;
+    g.gz = R;
+    g.px = ((nx + 2 * g.gx + e32 - 1) / e32) * e32;
+    g.py = ny + 2 * R;
+    g.pz = g.nz + 2 * R;
+    g.n = (long long)nx * ny * g.nz;
+    long long fs = (long long)g.px * g.py * g.pz;
+    const long long e256 = (long long)(256 / esize);
+    g.fs = ((fs + e256 - 1) / e256) * e256;
+    return g;
+}
+
+static bool pair_ok(const fd_ctx* c) { return c->dtype == FD_F32 && c->nz % 2 == 0 && c->nz / 2 >= 4; }
 
 // ------------------------------------------------------------------------------------------------
 // launch helpers (typed)
@@ -196,19 +261,22 @@ static int launch_halo(fd_ctx* c, T* F, int nfields) {
 
 // One substep of the selected path: F[cur] (valid ghosts) -> F[1-cur] (+ghosts if write_f), w updated.
 template <class T>
-static int launch_substep(fd_ctx* c, const Sub<T>& s) {
+static int launch_substep(fd_ctx* c, const SubD& sd) {
     const Geom& g = c->g;
     const Coef<T> k = make_coef<T>(c);
+    Sub<T> s = make_sub<T>(sd);
     const T* Fin = (const T*)c->F[c->cur];
     T* Fout = (T*)c->F[1 - c->cur];
     T* W = (T*)c->W;
     T* Div = (T*)c->Div;
     const bool p55 = c->path == FD_PATH_55;
+    const bool tiled = c->variant == FD_VARIANT_TILED || c->variant == FD_VARIANT_PAIRED;
     dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
     {
         LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
-        if (c->variant == FD_VARIANT_TILED) {
-            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, c->dx, c->nu, c->cs, s, c->stream))
+        if (tiled) {
+            const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w);
+            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, c->stream))
                 return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (p55) {
             k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
@@ -219,6 +287,7 @@ static int launch_substep(fd_ctx* c, const Sub<T>& s) {
     if (!p55) {
         int rc = launch_halo<T>(c, Div, 1);  // "Compute boundary conditions for (div u)" (Alg. 3)
         if (rc) return rc;
+        if (tiled) s.dt = T(typename Scalar<T>::type(1));  // the tiled pass 1 leaves dt * div u in Div
         LaunchScope ls(c, FD_K_PASS2);
         k_direct_pass2<T><<<grid, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
     }
@@ -235,21 +304,23 @@ template <class T>
 static int do_rk3(fd_ctx* c, double dt, int nsteps) {
     for (int n = 0; n < nsteps; ++n)
         for (int s = 0; s < 3; ++s) {
-            Sub<T> sub;
-            sub.alpha = T(kAlpha[s]);
-            sub.beta = T(kBeta[s]);
-            sub.dt = T(dt);
+            SubD sub;
+            sub.alpha = kAlpha[s];
+            sub.beta = kBeta[s];
+            sub.dt = dt;
             sub.read_w = s != 0;   // alpha^(1) = 0: w is not read
             sub.write_w = s != 2;  // ... so the w of the last substep is never read either: not written
             sub.write_f = 1;
             int rc = launch_substep<T>(c, sub);
             if (rc) return rc;
         }
+    if (nsteps > 0) c->loaded = true;
     return FD_OK;
 }
 
+// dense caller-layout arrays (4 x N scalars at src) -> F[cur] interior, then ghosts
 template <class T>
-static int do_pack(fd_ctx* c, const T* const src[4]) {
+static int do_pack(fd_ctx* c, const typename Scalar<T>::type* const src[4]) {
     const Geom& g = c->g;
     T* F = (T*)c->F[c->cur];
     {
@@ -261,9 +332,9 @@ static int do_pack(fd_ctx* c, const T* const src[4]) {
     return launch_halo<T>(c, F, 4);
 }
 
+// padded (or, with the dense geometry of the w arrays, dense) values -> dense caller-layout arrays
 template <class T>
-static int do_unpack(fd_ctx* c, const T* F, T* const dst[4]) {
-    const Geom& g = c->g;
+static int do_unpack(fd_ctx* c, const T* F, const Geom& g, typename Scalar<T>::type* const dst[4]) {
     LaunchScope ls(c, FD_K_UNPACK);
     dim3 grid((g.nx + 127) / 128, g.ny, g.nz * 4);
     k_unpack<T><<<grid, 128, 0, c->stream>>>(F, dst[0], dst[1], dst[2], dst[3], g);
@@ -271,75 +342,132 @@ static int do_unpack(fd_ctx* c, const T* F, T* const dst[4]) {
     return FD_OK;
 }
 
+static Geom dense_geom(const Geom& g) {  // the w arrays seen as "padded" arrays without ghosts
+    Geom d = g;
+    d.px = g.nx;
+    d.py = g.ny;
+    d.pz = g.nz;
+    d.gx = d.gy = d.gz = 0;
+    d.fs = g.n;
+    return d;
+}
+
 template <class T>
 static int do_load(fd_ctx* c, const void* const in[4], int where) {
-    const size_t nb = (size_t)c->g.n * sizeof(T);
-    const T* src[4];
+    typedef typename Scalar<T>::type S;
+    const size_t nscal = (size_t)c->nx * c->ny * c->nz;
+    const size_t nb = nscal * sizeof(S);
+    const S* src[4];
     for (int q = 0; q < 4; ++q) {
         if (where == FD_HOST) {
-            T* stage = (T*)c->W + (size_t)q * c->g.n;  // w is scratch between steps (alpha_1 = 0)
+            S* stage = (S*)c->W + (size_t)q * nscal;  // w is scratch between steps (alpha_1 = 0)
             FD_CUDA(cudaMemcpyAsync(stage, in[q], nb, cudaMemcpyHostToDevice, c->stream));
             src[q] = stage;
         } else {
-            src[q] = (const T*)in[q];
+            src[q] = (const S*)in[q];
         }
     }
     int rc = do_pack<T>(c, src);
     if (rc) return rc;
+    c->loaded = true;
     if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
     return FD_OK;
 }
 
-template <class T>
-static int copy_out(fd_ctx* c, const T* dense_w, void* const out[4]) {
-    // dense_w: four dense arrays in W, to the caller's host arrays.
-    const size_t nb = (size_t)c->g.n * sizeof(T);
+// four dense caller-layout arrays at `dense` (device) -> the caller's host arrays
+template <class S>
+static int copy_out(fd_ctx* c, const S* dense, void* const out[4]) {
+    const size_t nscal = (size_t)c->nx * c->ny * c->nz;
     for (int q = 0; q < 4; ++q)
-        FD_CUDA(cudaMemcpyAsync(out[q], dense_w + (size_t)q * c->g.n, nb, cudaMemcpyDeviceToHost, c->stream));
+        FD_CUDA(cudaMemcpyAsync(out[q], dense + (size_t)q * nscal, nscal * sizeof(S), cudaMemcpyDeviceToHost, c->stream));
     FD_CUDA(cudaStreamSynchronize(c->stream));
     return FD_OK;
 }
 
 template <class T>
 static int do_store(fd_ctx* c, void* const out[4], int where) {
-    T* dst[4];
-    for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (T*)c->W + (size_t)q * c->g.n : (T*)out[q];
-    int rc = do_unpack<T>(c, (const T*)c->F[c->cur], dst);
+    typedef typename Scalar<T>::type S;
+    const size_t nscal = (size_t)c->nx * c->ny * c->nz;
+    S* dst[4];
+    for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (S*)c->W + (size_t)q * nscal : (S*)out[q];
+    int rc = do_unpack<T>(c, (const T*)c->F[c->cur], c->g, dst);
     if (rc) return rc;
-    return where == FD_HOST ? copy_out<T>(c, (const T*)c->W, out) : FD_OK;
+    return where == FD_HOST ? copy_out<S>(c, (const S*)c->W, out) : FD_OK;
 }
 
 template <class T>
 static int do_rhs(fd_ctx* c, void* const out[4], int where) {
-    Sub<T> sub;
-    sub.alpha = T(0);
-    sub.beta = T(0);
-    sub.dt = T(1);
+    typedef typename Scalar<T>::type S;
+    SubD sub;
+    sub.alpha = 0;
+    sub.beta = 0;
+    sub.dt = 1;
     sub.read_w = 0;
     sub.write_w = 1;
     sub.write_f = 0;  // w <- rhs, state untouched
     int rc = launch_substep<T>(c, sub);
     if (rc) return rc;
-    const size_t nb = (size_t)c->g.n * sizeof(T);
-    for (int q = 0; q < 4; ++q)
-        FD_CUDA(cudaMemcpyAsync(out[q], (const T*)c->W + (size_t)q * c->g.n, nb,
-                                where == FD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
-    if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
-    return FD_OK;
+    const size_t nscal = (size_t)c->nx * c->ny * c->nz;
+    if (Scalar<T>::lanes == 1) {  // the w arrays already are in the caller's layout
+        for (int q = 0; q < 4; ++q)
+            FD_CUDA(cudaMemcpyAsync(out[q], (const S*)c->W + (size_t)q * nscal, nscal * sizeof(S),
+                                    where == FD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+        if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
+        return FD_OK;
+    }
+    // paired layout: un-pair w; the write copy of the fields is free scratch for the host staging
+    S* dst[4];
+    for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (S*)c->F[1 - c->cur] + (size_t)q * nscal : (S*)out[q];
+    rc = do_unpack<T>(c, (const T*)c->W, dense_geom(c->g), dst);
+    if (rc) return rc;
+    return where == FD_HOST ? copy_out<S>(c, (const S*)c->F[1 - c->cur], out) : FD_OK;
+}
+
+// Switch between the plain and the paired layout, carrying a loaded state across through the w scratch.
+static int set_layout(fd_ctx* c, bool paired) {
+    if (paired == c->paired) return FD_OK;
+    const size_t nscal = (size_t)c->nx * c->ny * c->nz;
+    void* dense[4];
+    for (int q = 0; q < 4; ++q) dense[q] = (char*)c->W + (size_t)q * nscal * 4;  // fp32 only
+    int rc = FD_OK;
+    if (c->loaded) {
+        rc = FD_DISPATCH(c, do_store<T>(c, dense, FD_DEVICE));
+        if (rc) return rc;
+    }
+    c->paired = paired;
+    c->esize = paired ? 8 : 4;
+    c->g = make_geom(c->nx, c->ny, c->nz, c->esize, paired);
+    // ghost cells of the other layout are interior cells of this one: start both copies from zero again
+    FD_CUDA(cudaMemsetAsync(c->F[1 - c->cur], 0, c->f_bytes, c->stream));
+    if (c->Div) FD_CUDA(cudaMemsetAsync(c->Div, 0, c->div_bytes, c->stream));
+    if (c->loaded) {
+        FD_CUDA(cudaMemsetAsync(c->F[c->cur], 0, c->f_bytes, c->stream));
+        rc = FD_DISPATCH(c, do_load<T>(c, (const void* const*)dense, FD_DEVICE));
+    }
+    return rc;
 }
 
 static int resolve_variant(fd_ctx* c) {
     int want = c->variant_req;
-    bool tiled_ok = tiled_supported(c->g, c->dtype);
-    if (want == FD_VARIANT_AUTO) want = tiled_ok ? FD_VARIANT_TILED : FD_VARIANT_DIRECT;
-    if (want == FD_VARIANT_TILED) {
-        if (!tiled_ok) return fail(FD_EUNSUPPORTED, "tiled variant does not support this grid");
-        int rc = tiled_prepare(c->tiled, c->g, c->dtype, c->F[0], c->F[1], c->Div);
+    if (want == FD_VARIANT_AUTO) want = pair_ok(c) ? FD_VARIANT_PAIRED : FD_VARIANT_TILED;
+    if (want == FD_VARIANT_PAIRED && !pair_ok(c)) {
+        if (c->variant_req != FD_VARIANT_AUTO)
+            return fail(FD_EUNSUPPORTED, "paired variant needs fp32 and an even nz >= 8 (got dtype %d, nz %d)", c->dtype, c->nz);
+        want = FD_VARIANT_TILED;
+    }
+    // layout: the paired variant needs the paired layout, the plain tiled one the plain layout; direct runs on either
+    int rc = FD_OK;
+    if (want == FD_VARIANT_PAIRED) rc = set_layout(c, true);
+    if (want == FD_VARIANT_TILED) rc = set_layout(c, false);
+    if (rc) return rc;
+    if (want == FD_VARIANT_TILED || want == FD_VARIANT_PAIRED) {
+        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1])) : 4;
         if (rc != FD_OK) {
             if (c->variant_req == FD_VARIANT_AUTO) {
                 want = FD_VARIANT_DIRECT;
             } else {
-                return fail(rc, "tiled variant setup failed: %s", tiled_error_of(c->tiled));
+                return fail(rc == 4 ? FD_EUNSUPPORTED : FD_ECUDA, "tiled variant setup failed: %s",
+                            rc == 4 ? "grid too small" : tiled_error_of(c->tiled));
             }
         }
     }
@@ -374,38 +502,36 @@ extern "C" int fd_create(fd_ctx** out, int nx, int ny, int nz, double dx, double
     fd_ctx* c = new (std::nothrow) fd_ctx();
     if (!c) return fail(FD_ENOMEM, "fd_create: host allocation failed");
     c->dtype = dtype;
-    c->esize = dtype == FD_F32 ? 4 : 8;
+    c->nx = nx;
+    c->ny = ny;
+    c->nz = nz;
     c->dx = dx;
     c->nu = nu;
     c->cs = cs;
     c->alloc = g_alloc;
     c->release = g_free;
     c->alloc_user = g_alloc_user;
-    // HBM layout: 32-byte ghost pad in x so interior rows start sector-aligned and 16-byte vector /
-    // TMA accesses are legal; row pitch a multiple of 32 bytes; 3 ghost rows / planes in y and z.
-    Geom& g = c->g;
-    const int e32 = (int)(32 / c->esize);
-    g.nx = nx;
-    g.ny = ny;
-    g.nz = nz;
-    g.gx = e32;
-    g.gy = R;
-    g.gz = R;
-    g.px = ((nx + 2 * g.gx + e32 - 1) / e32) * e32;
-    g.py = ny + 2 * R;
-    g.pz = nz + 2 * R;
-    g.n = (long long)nx * ny * nz;
-    long long fs = (long long)g.px * g.py * g.pz;
-    const long long e256 = (long long)(256 / c->esize);
-    g.fs = ((fs + e256 - 1) / e256) * e256;
+    // The context starts in the plain layout; resolve_variant switches fp32 grids with an even nz to the paired
+    // one.  The buffers are sized for whichever of the two layouts is larger.
+    c->paired = false;
+    c->esize = dtype == FD_F32 ? 4 : 8;
+    c->g = make_geom(nx, ny, nz, c->esize, false);
+    c->f_bytes = (size_t)c->g.fs * 4 * c->esize;
+    c->div_bytes = (size_t)c->g.fs * c->esize;
+    if (pair_ok(c)) {
+        const Geom gp = make_geom(nx, ny, nz, 8, true);
+        if ((size_t)gp.fs * 4 * 8 > c->f_bytes) c->f_bytes = (size_t)gp.fs * 4 * 8;
+        if ((size_t)gp.fs * 8 > c->div_bytes) c->div_bytes = (size_t)gp.fs * 8;
+    }
+    const size_t w_bytes = (size_t)nx * ny * nz * 4 * (dtype == FD_F32 ? 4 : 8);
     int rc = FD_OK;
     for (int b = 0; b < 2 && rc == FD_OK; ++b) {
-        rc = ctx_alloc(c, &c->F[b], (size_t)g.fs * 4 * c->esize);
-        if (rc == FD_OK && cudaMemsetAsync(c->F[b], 0, (size_t)g.fs * 4 * c->esize, c->stream) != cudaSuccess)
+        rc = ctx_alloc(c, &c->F[b], c->f_bytes);
+        if (rc == FD_OK && cudaMemsetAsync(c->F[b], 0, c->f_bytes, c->stream) != cudaSuccess)
             rc = fail(FD_ECUDA, "fd_create: memset failed: %s", cudaGetErrorString(cudaGetLastError()));
     }
-    if (rc == FD_OK) rc = ctx_alloc(c, &c->W, (size_t)g.n * 4 * c->esize);
-    if (rc == FD_OK && cudaMemsetAsync(c->W, 0, (size_t)g.n * 4 * c->esize, c->stream) != cudaSuccess)
+    if (rc == FD_OK) rc = ctx_alloc(c, &c->W, w_bytes);
+    if (rc == FD_OK && cudaMemsetAsync(c->W, 0, w_bytes, c->stream) != cudaSuccess)
         rc = fail(FD_ECUDA, "fd_create: memset failed: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc == FD_OK) rc = resolve_variant(c);
     if (rc != FD_OK) {
@@ -441,11 +567,9 @@ extern "C" int fd_set_path(fd_ctx* c, int path) {
     FD_CHECK_CTX(c);
     if (path != FD_PATH_55 && path != FD_PATH_19) return fail(FD_EINVAL, "fd_set_path: bad path %d", path);
     if (path == FD_PATH_19 && !c->Div) {
-        int rc = ctx_alloc(c, &c->Div, (size_t)c->g.fs * c->esize);
+        int rc = ctx_alloc(c, &c->Div, c->div_bytes);
         if (rc) return rc;
-        FD_CUDA(cudaMemsetAsync(c->Div, 0, (size_t)c->g.fs * c->esize, c->stream));
-        c->path = path;
-        return resolve_variant(c);  // the tiled variant needs a tensor map of the div array
+        FD_CUDA(cudaMemsetAsync(c->Div, 0, c->div_bytes, c->stream));
     }
     c->path = path;
     return FD_OK;
@@ -453,7 +577,7 @@ extern "C" int fd_set_path(fd_ctx* c, int path) {
 
 extern "C" int fd_set_variant(fd_ctx* c, int variant) {
     FD_CHECK_CTX(c);
-    if (variant < FD_VARIANT_AUTO || variant > FD_VARIANT_TILED) return fail(FD_EINVAL, "fd_set_variant: bad variant %d", variant);
+    if (variant < FD_VARIANT_AUTO || variant > FD_VARIANT_PAIRED) return fail(FD_EINVAL, "fd_set_variant: bad variant %d", variant);
     int old = c->variant_req;
     c->variant_req = variant;
     int rc = resolve_variant(c);
@@ -483,7 +607,7 @@ extern "C" int fd_load(fd_ctx* c, const void* lnrho, const void* ux, const void*
     int rc = check_ptrs("fd_load", lnrho, ux, uy, uz, where);
     if (rc) return rc;
     const void* in[4] = {lnrho, ux, uy, uz};
-    return c->dtype == FD_F32 ? do_load<float>(c, in, where) : do_load<double>(c, in, where);
+    return FD_DISPATCH(c, do_load<T>(c, in, where));
 }
 
 extern "C" int fd_store(fd_ctx* c, void* lnrho, void* ux, void* uy, void* uz, int where) {
@@ -491,7 +615,7 @@ extern "C" int fd_store(fd_ctx* c, void* lnrho, void* ux, void* uy, void* uz, in
     int rc = check_ptrs("fd_store", lnrho, ux, uy, uz, where);
     if (rc) return rc;
     void* out[4] = {lnrho, ux, uy, uz};
-    return c->dtype == FD_F32 ? do_store<float>(c, out, where) : do_store<double>(c, out, where);
+    return FD_DISPATCH(c, do_store<T>(c, out, where));
 }
 
 extern "C" int fd_rhs(fd_ctx* c, void* r0, void* r1, void* r2, void* r3, int where) {
@@ -499,14 +623,14 @@ extern "C" int fd_rhs(fd_ctx* c, void* r0, void* r1, void* r2, void* r3, int whe
     int rc = check_ptrs("fd_rhs", r0, r1, r2, r3, where);
     if (rc) return rc;
     void* out[4] = {r0, r1, r2, r3};
-    return c->dtype == FD_F32 ? do_rhs<float>(c, out, where) : do_rhs<double>(c, out, where);
+    return FD_DISPATCH(c, do_rhs<T>(c, out, where));
 }
 
 extern "C" int fd_rk3_step(fd_ctx* c, double dt, int nsteps) {
     FD_CHECK_CTX(c);
     if (nsteps < 0) return fail(FD_EINVAL, "fd_rk3_step: nsteps < 0");
     if (!std::isfinite(dt)) return fail(FD_EINVAL, "fd_rk3_step: dt is not finite");
-    return c->dtype == FD_F32 ? do_rk3<float>(c, dt, nsteps) : do_rk3<double>(c, dt, nsteps);
+    return FD_DISPATCH(c, do_rk3<T>(c, dt, nsteps));
 }
 
 extern "C" int fd_sync(fd_ctx* c) {
@@ -520,9 +644,9 @@ extern "C" int fd_get_info(const fd_ctx* c, fd_info* o) {
     FD_CHECK_CTX(c);
     if (!o) return fail(FD_EINVAL, "fd_get_info: out is NULL");
     const Geom& g = c->g;
-    o->nx = g.nx;
-    o->ny = g.ny;
-    o->nz = g.nz;
+    o->nx = c->nx;
+    o->ny = c->ny;
+    o->nz = c->nz;
     o->dtype = c->dtype;
     o->path = c->path;
     o->variant = c->variant;
@@ -572,8 +696,9 @@ extern "C" int fd_reset_profile(fd_ctx* c) {
 
 template <class T>
 static int do_poison(fd_ctx* c, bool ghosts) {
-    const T nan = T(NAN);
+    const T nan = T(typename Scalar<T>::type(NAN));
     if (ghosts) {
+        c->loaded = true;  // the zero state is gone: a layout switch must carry the fields across
         long long n = (long long)c->g.px * c->g.py * c->g.pz * 4;
         for (int b = 0; b < 2; ++b) {
             c->launches++;
@@ -590,10 +715,10 @@ static int do_poison(fd_ctx* c, bool ghosts) {
 
 extern "C" int fd_debug_poison_w(fd_ctx* c) {
     FD_CHECK_CTX(c);
-    return c->dtype == FD_F32 ? do_poison<float>(c, false) : do_poison<double>(c, false);
+    return FD_DISPATCH(c, do_poison<T>(c, false));
 }
 
 extern "C" int fd_debug_poison_ghosts(fd_ctx* c) {
     FD_CHECK_CTX(c);
-    return c->dtype == FD_F32 ? do_poison<float>(c, true) : do_poison<double>(c, true);
+    return FD_DISPATCH(c, do_poison<T>(c, true));
 }

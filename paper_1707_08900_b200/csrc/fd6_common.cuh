@@ -10,8 +10,51 @@ namespace fd6 {
 
 constexpr int R = 3;  // stencil radius, "For both stencils, R = 3"
 
-// Ghost-padded array geometry.  Cell (i,j,k) of a padded field lives at
-//   (i + gx) + px * ((j + gy) + py * (k + gz));  the four fields of one copy are fs elements apart.
+// ------------------------------------------------------------------------------------------------
+// V2 — two fp32 cells in one 64-bit value.  In the paired layout cell
+// (i,j,k) and cell (i,j,k+nz/2) are stored side by side, so every kernel sees a grid of nz/2 planes whose
+// elements are V2, and the arithmetic on both cells is ONE packed instruction (Blackwell FFMA2 / FADD2 /
+// FMUL2: fma.rn.f32x2 etc., PTX ISA 8.6, sm_100) with both halves rounded exactly like the scalar op.
+// ------------------------------------------------------------------------------------------------
+struct __align__(8) V2 {
+    float2 v;
+    V2() = default;
+    __host__ __device__ explicit V2(float s) : v{s, s} {}
+    __host__ __device__ explicit V2(double s) : v{(float)s, (float)s} {}
+    __host__ __device__ explicit V2(int s) : v{(float)s, (float)s} {}
+    __host__ __device__ V2(float lo, float hi) : v{lo, hi} {}
+};
+__device__ __forceinline__ V2 mk(float2 f) {
+    V2 r;
+    r.v = f;
+    return r;
+}
+__device__ __forceinline__ V2 operator+(V2 a, V2 b) { return mk(__fadd2_rn(a.v, b.v)); }
+__device__ __forceinline__ V2 operator-(V2 a) { return V2(-a.v.x, -a.v.y); }
+__device__ __forceinline__ V2 operator-(V2 a, V2 b) { return mk(__fadd2_rn(a.v, make_float2(-b.v.x, -b.v.y))); }
+__device__ __forceinline__ V2 operator*(V2 a, V2 b) { return mk(__fmul2_rn(a.v, b.v)); }
+__device__ __forceinline__ V2& operator+=(V2& a, V2 b) { return a = a + b; }
+__device__ __forceinline__ V2& operator-=(V2& a, V2 b) { return a = a - b; }
+
+// fma_(a, b, c) = a*b + c with one rounding, for every value type the kernels are instantiated on.
+__device__ __forceinline__ float fma_(float a, float b, float c) { return fmaf(a, b, c); }
+__device__ __forceinline__ double fma_(double a, double b, double c) { return fma(a, b, c); }
+__device__ __forceinline__ V2 fma_(V2 a, V2 b, V2 c) { return mk(__ffma2_rn(a.v, b.v, c.v)); }
+
+// Periodic wrap across the z boundary of the stored grid: in the paired layout the plane below plane 0 is
+// plane nz/2-1 of the OTHER half, so the two halves of every value trade places; scalars are unchanged.
+template <class T>
+__device__ __forceinline__ T zwrap(T v) { return v; }
+template <>
+__device__ __forceinline__ V2 zwrap<V2>(V2 v) { return V2(v.v.y, v.v.x); }
+
+// Scalar type behind a value type, and cells per value.
+template <class T> struct Scalar { typedef T type; static constexpr int lanes = 1; };
+template <> struct Scalar<V2> { typedef float type; static constexpr int lanes = 2; };
+
+// Ghost-padded array geometry, in units of the value type T of the kernels (one cell,
+// or a V2 pair of cells: then nz is HALF the caller's nz).  Value (i,j,k) of a padded field lives at
+//   (i + gx) + px * ((j + gy) + py * (k + gz));  the four fields of one copy are fs values apart.
 struct Geom {
     int nx, ny, nz;
     int px, py, pz;

@@ -10,28 +10,50 @@ namespace fd6 {
 // a0  pack / unpack: caller's dense arrays <-> interior of the padded arrays.
 // grid (ceil(nx/128), ny, nz) x 4 fields through blockIdx.z = k + nz*q.
 // ------------------------------------------------------------------------------------------------
+// Dense caller arrays hold scalars; in the paired layout value (i,j,k) gathers cells k and k + g.nz.
 template <class T>
-__global__ void __launch_bounds__(128) k_pack(const T* __restrict__ d0, const T* __restrict__ d1_, const T* __restrict__ d2_,
-                                              const T* __restrict__ d3, T* __restrict__ F, Geom g) {
-    int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z % g.nz, q = blockIdx.z / g.nz;
-    if (i >= g.nx) return;
-    const T* src = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
-    F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))] =
-        src[i + (long long)g.nx * (j + (long long)g.ny * k)];
+__device__ __forceinline__ T dense_get(const typename Scalar<T>::type* __restrict__ a, long long idx, long long half) {
+    return a[idx];
+}
+template <>
+__device__ __forceinline__ V2 dense_get<V2>(const float* __restrict__ a, long long idx, long long half) {
+    return V2(a[idx], a[idx + half]);
+}
+template <class T>
+__device__ __forceinline__ void dense_put(typename Scalar<T>::type* __restrict__ a, long long idx, long long half, T v) {
+    a[idx] = v;
+}
+template <>
+__device__ __forceinline__ void dense_put<V2>(float* __restrict__ a, long long idx, long long half, V2 v) {
+    a[idx] = v.v.x;
+    a[idx + half] = v.v.y;
 }
 
 template <class T>
-__global__ void __launch_bounds__(128) k_unpack(const T* __restrict__ F, T* __restrict__ d0, T* __restrict__ d1_,
-                                                T* __restrict__ d2_, T* __restrict__ d3, Geom g) {
+__global__ void __launch_bounds__(128)
+    k_pack(const typename Scalar<T>::type* __restrict__ d0, const typename Scalar<T>::type* __restrict__ d1_,
+           const typename Scalar<T>::type* __restrict__ d2_, const typename Scalar<T>::type* __restrict__ d3, T* __restrict__ F, Geom g) {
     int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z % g.nz, q = blockIdx.z / g.nz;
     if (i >= g.nx) return;
-    T* dst = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
-    dst[i + (long long)g.nx * (j + (long long)g.ny * k)] =
-        F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))];
+    const typename Scalar<T>::type* src = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
+    F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))] =
+        dense_get<T>(src, i + (long long)g.nx * (j + (long long)g.ny * k), g.n);
+}
+
+template <class T>
+__global__ void __launch_bounds__(128)
+    k_unpack(const T* __restrict__ F, typename Scalar<T>::type* __restrict__ d0, typename Scalar<T>::type* __restrict__ d1_,
+             typename Scalar<T>::type* __restrict__ d2_, typename Scalar<T>::type* __restrict__ d3, Geom g) {
+    int i = blockIdx.x * 128 + threadIdx.x, j = blockIdx.y, k = blockIdx.z % g.nz, q = blockIdx.z / g.nz;
+    if (i >= g.nx) return;
+    typename Scalar<T>::type* dst = q == 0 ? d0 : (q == 1 ? d1_ : (q == 2 ? d2_ : d3));
+    dense_put<T>(dst, i + (long long)g.nx * (j + (long long)g.ny * k), g.n,
+                 F[q * g.fs + (i + g.gx) + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz))]);
 }
 
 // ------------------------------------------------------------------------------------------------
 // a1 / a7  periodic halo fill, radius 3 (Alg. 2/3 "Compute boundary conditions").
+//   (T = V2: the stored grid has nz/2 planes and z-periodicity swaps the halves of a pair, see zwrap.)
 //   k_halo_x : every interior row (j,k) copies 3 cells to each x ghost.          thread per (row, field)
 //   k_halo_yz: every ghost ROW (j or k outside the domain) is the x-extended copy of the interior row it
 //              wraps to; run after k_halo_x so edge ghosts (two coordinates outside, needed by the Eq. 8
@@ -69,15 +91,20 @@ __global__ void __launch_bounds__(128) k_halo_yz(T* __restrict__ F, Geom g) {
         kk = k + g.gz;
         jj = yr < R ? yr + (g.gy - R) : g.gy + g.ny + (yr - R);
     }
-    int js = jj - g.gy, ks = kk - g.gz;  // wrap to the interior row (n >= 8 > R: one correction suffices)
+    int js = jj - g.gy, ks = kk - g.gz;  // wrap to the interior row (n >= R: one correction suffices)
     js += js < 0 ? g.ny : 0;
     js -= js >= g.ny ? g.ny : 0;
+    const bool zw = ks < 0 || ks >= g.nz;  // paired layout: crossing the z boundary swaps the two halves
     ks += ks < 0 ? g.nz : 0;
     ks -= ks >= g.nz ? g.nz : 0;
     T* base = F + blockIdx.y * g.fs;
     T* dst = base + (long long)g.px * (jj + (long long)g.py * kk) + (g.gx - R);
     const T* src = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz)) + (g.gx - R);
-    for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = src[x];
+    if (zw) {
+        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = zwrap<T>(src[x]);
+    } else {
+        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = src[x];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------

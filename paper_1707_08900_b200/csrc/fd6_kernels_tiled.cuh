@@ -1,20 +1,24 @@
-// fd6_kernels_tiled.cuh — FD_VARIANT_TILED: the fast derivative/update kernel.
+// fd6_kernels_tiled.cuh — FD_VARIANT_TILED / FD_VARIANT_PAIRED: the fast derivative/update kernel
+// (DESIGN.md "Kernels").  One template, three value types: float, double, and V2 (two fp32 cells per value,
+// packed FFMA2/FADD2/FMUL2 arithmetic — the paired layout).
 //
-// One CTA owns a TX x TY column of cells and marches along z through a chunk of planes.  A plane of all four
+// One CTA owns a TX x TY column of values and marches along z through a chunk of planes.  A plane of all four
 // fields plus its radius-3 halo is staged into shared memory by ONE 4-D TMA box copy (cp.async.bulk.tensor,
-// mbarrier complete_tx), four stages deep, so a plane is read from L2/HBM once per CTA.  Each thread owns one
-// cell column and keeps everything that couples planes in registers:
-//   win[f][8]   sliding window of its own cell's values along z           -> D1z, D2z             (Eq. 6, 7)
-//   dl[q][4]    the in-plane first derivatives of the last planes, delayed until the plane is the centre
-//   lin[i][8]   accumulator ring of the part of the right-hand side that is LINEAR in second derivatives,
-//               nu (lap u_i + 1/3 d_i div u): in-plane D2x, D2y, Dxy are added when the plane is staged, and the
-//               mixed derivatives that involve z (Eq. 8) are formed from the in-plane differences
+// mbarrier complete_tx) through an NS-deep ring of stages; a stage is handed back to the TMA producer through a
+// second ("empty") mbarrier on which every warp arrives once it has read the plane, so there is no CTA-wide
+// barrier in the loop.  Each thread owns one column and keeps everything that couples planes in registers:
+//   win[f][8]   sliding window of its own column along z                     -> D1z, D2z          (Eq. 6, 7)
+//   lin[i][8]   accumulator ring of everything of dt*rhs_i that is known when a plane is staged: the in-plane
+//               second derivatives (D2x, D2y, Dxy), the in-plane part of the nonlinear terms, and the mixed
+//               derivatives that involve z (Eq. 8), which are formed from the in-plane differences
 //               f(x+m) - f(x-m) that D1x / D1y need anyway:  Dxz f(z) = sum_m c_m [dx_m f(z+m) - dx_m f(z-m)],
-//               so plane t scatters +-c_m dx_m into the ring slots of outputs t-m and t+m (no extra loads).
-// Output plane z = t-3 is assembled (Eq. 1-3) and updated (Eq. 10) when plane t = z+3 has been consumed.
+//               so plane t scatters +-c_m dx_m into the ring slots of outputs t-m and t+m (no extra loads)
+//   dl[6][4]    the six in-plane quantities that multiply z derivatives, delayed until their plane is the centre.
+// Output plane z = t-3 is finished (Eq. 1-3) and updated (Eq. 10) when plane t = z+3 has been consumed.
+// dt is folded into the velocity-derivative coefficients, so the kernel forms dt*rhs directly.
 // The accumulation order of every output depends only on relative plane index, never on the position in a
 // tile or chunk, so periodic-shift equivariance stays bitwise.
-// PATH55 = false is pass 1 of the 19-point path (no mixed derivatives, div u written, Eq. 14-16).
+// PATH55 = false is pass 1 of the 19-point path (no mixed derivatives, dt*div u written, Eq. 14-16).
 #pragma once
 #include <cuda.h>
 
@@ -22,15 +26,19 @@
 
 namespace fd6 {
 
-// Coefficients with the physics constants folded in (formed in double on the host, rounded once to T).
+// Coefficients with the physics constants, dt and the RK substep folded in (formed in double on the host,
+// rounded once to the scalar type; V2 holds the same number in both halves).
 template <class T>
-struct TCoef {
-    T a[3];    // Eq. 6:  a_m / (60 dx)
-    T lo[4];   // nu * b_m / (180 dx^2), m = 0..3          second derivative along an axis other than i
-    T lq[4];   // PATH55: (4 nu / 3) * b_m (d_ii u_i enters lap u_i and d_i div u);  PATH19: same as lo
-    T cxy[3];  // centre coefficient of the in-plane part for u_x, u_y, u_z
-    T mq[3];   // (nu / 3) * c_m / (720 dx^2)              Eq. 8
-    T nu, cs2, nu23;
+struct KC {
+    T ar[3];   // Eq. 6:  a_m / (60 dx)                     first derivatives of ln rho
+    T au[3];   // dt a_m / (60 dx)                          first derivatives of u (carry dt)
+    T lo[4];   // dt nu b_m / (180 dx^2), m = 0..3          second derivative along an axis other than i
+    T lq[4];   // PATH55: dt (4 nu / 3) b_m (d_ii u_i enters lap u_i and d_i div u);  PATH19: same as lo
+    T cxy[3];  // centre coefficient of the in-plane second derivatives of u_x, u_y, u_z
+    T mq[3];   // dt (nu / 3) c_m / (720 dx^2)              Eq. 8
+    T nu, nu2, nu23, cs2dt, dt;
+    T alpha, beta;
+    int read_w, write_f, write_w;
 };
 
 // ---- mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk.tensor) --------------------------------
@@ -40,6 +48,9 @@ __device__ __forceinline__ void mbar_init(uint64_t* b, uint32_t count) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* b, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
     asm volatile(
@@ -64,153 +75,199 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, ui
 
 template <class T, bool PATH55, int TX, int TY>
 struct Tiled {
-    static constexpr int PXS = TX + 8;  // staged row: 4 cells left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
+    static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
     static constexpr int PYS = TY + 2 * R;
     static constexpr int FIELD = PXS * PYS;
-    static constexpr int STAGE = 4 * FIELD;  // elements per stage: four fields of one plane
-    static constexpr int S = 4;              // stages (divides the unroll factor 8: stage offsets are immediates)
+    static constexpr int STAGE = 4 * FIELD;  // values per stage: four fields of one plane
+    static constexpr int NS = 8;             // stages = unroll factor of the plane loop: stage offsets are immediates
     static constexpr int THREADS = TX * TY;
-    static constexpr size_t SMEM = (size_t)S * STAGE * sizeof(T) + S * sizeof(uint64_t);
+    static constexpr int WARPS = THREADS / 32;
+    static constexpr size_t SMEM = (size_t)NS * STAGE * sizeof(T) + 2 * NS * sizeof(uint64_t);
 
     struct State {
         T win[4][8];
         T lin[3][8];
-        T dl[8][4];
+        T dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 — of the last planes
     };
 
     template <int PH>
-    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const TCoef<T>& c, const Sub<T>& s, int p,
-                                                bool store_ok, const T* __restrict__ wp, T* __restrict__ wq, T* __restrict__ fo,
-                                                T* __restrict__ dv, long long fs, long long n) {
+    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const KC<T>& c, int p, bool store_ok,
+                                                const T* __restrict__ wp, T* __restrict__ wq, T* __restrict__ fo, T* __restrict__ dv,
+                                                long long fs, long long n) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
-        const T* sp = sp0 + n4 * STAGE;
+        const T* sp = sp0 + n8 * STAGE;
         const bool out = p >= 2 * R;  // planes 0..5 of a chunk only warm the window and the rings up
         T wold[4];
-        if (out && s.read_w) {
+        if (out && c.read_w) {
 #pragma unroll
             for (int f = 0; f < 4; ++f) wold[f] = store_ok ? wp[f * n] : T(0);
         }
-        T inpl[3];                      // in-plane part of nu (lap u_i + 1/3 d_i div u) at the staged plane
-        T dgx = T(0), dgy = T(0);       // nu/3 d_xy u_y -> component x, nu/3 d_xy u_x -> component y
-        T ex[3], ey[3], ez[3];          // the differences that feed Dxz u_z, Dyz u_z, Dzx u_x + Dzy u_y
+        // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8)
+        T ctr[4], d1x[4], d1y[4], inpl[3];
+        T ex[3], ey[3], ez[3];  // the differences that feed Dxz u_z, Dyz u_z, Dzx u_x + Dzy u_y
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
             const T* q = sp + f * FIELD;
-            const T ctr = q[0];
-            st.win[f][n8] = ctr;
+            ctr[f] = q[0];
+            st.win[f][n8] = ctr[f];
             const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
             const T yp1 = q[PXS], ym1 = q[-PXS], yp2 = q[2 * PXS], ym2 = q[-2 * PXS], yp3 = q[3 * PXS], ym3 = q[-3 * PXS];
             const T dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
             const T dy1 = yp1 - ym1, dy2 = yp2 - ym2, dy3 = yp3 - ym3;
-            st.dl[2 * f][n4] = c.a[0] * dx1 + c.a[1] * dx2 + c.a[2] * dx3;
-            st.dl[2 * f + 1][n4] = c.a[0] * dy1 + c.a[1] * dy2 + c.a[2] * dy3;
+            const T* a = f == 0 ? c.ar : c.au;
+            d1x[f] = fma_(a[2], dx3, fma_(a[1], dx2, a[0] * dx1));
+            d1y[f] = fma_(a[2], dy3, fma_(a[1], dy2, a[0] * dy1));
             if (f > 0) {
                 const T sx1 = xp1 + xm1, sx2 = xp2 + xm2, sx3 = xp3 + xm3;
                 const T sy1 = yp1 + ym1, sy2 = yp2 + ym2, sy3 = yp3 + ym3;
                 const T* bx = f == 1 ? c.lq : c.lo;  // d_xx u_x and d_yy u_y carry 4nu/3 on the 55-point path
                 const T* by = f == 2 ? c.lq : c.lo;
-                inpl[f - 1] = c.cxy[f - 1] * ctr + bx[1] * sx1 + bx[2] * sx2 + bx[3] * sx3 + by[1] * sy1 + by[2] * sy2 + by[3] * sy3;
+                T v = c.cxy[f - 1] * ctr[f];
+                v = fma_(bx[1], sx1, v);
+                v = fma_(by[1], sy1, v);
+                v = fma_(bx[2], sx2, v);
+                v = fma_(by[2], sy2, v);
+                v = fma_(bx[3], sx3, v);
+                v = fma_(by[3], sy3, v);
+                if (PATH55 && (f == 1 || f == 2)) {  // Eq. 8 in the xy plane: d_xy u_x -> rhs_y, d_xy u_y -> rhs_x
+                    const T q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
+                    const T q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
+                    const T q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
+                    const T dq = fma_(c.mq[2], q3, fma_(c.mq[1], q2, c.mq[0] * q1));
+                    if (f == 1) { inpl[0] = v; inpl[1] = dq; } else { inpl[1] += v; inpl[0] += dq; }
+                } else {
+                    inpl[f - 1] = v;
+                }
             }
             if (PATH55) {
                 if (f == 1) { ez[0] = dx1; ez[1] = dx2; ez[2] = dx3; }
                 if (f == 2) { ez[0] += dy1; ez[1] += dy2; ez[2] += dy3; }
                 if (f == 3) { ex[0] = dx1; ex[1] = dx2; ex[2] = dx3; ey[0] = dy1; ey[1] = dy2; ey[2] = dy3; }
-                if (f == 1 || f == 2) {  // Eq. 8 in the xy plane: d_xy u_x -> (grad div)_y, d_xy u_y -> (grad div)_x
-                    const T q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
-                    const T q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
-                    const T q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
-                    const T dq = c.mq[0] * q1 + c.mq[1] * q2 + c.mq[2] * q3;
-                    if (f == 1) dgy = dq; else dgx = dq;
-                }
             }
         }
-        if (PATH55) {
-            inpl[0] += dgx;
-            inpl[1] += dgy;
-            const T* e[3] = {ex, ey, ez};
+        // ---- plane t: everything of dt*rhs that needs no z derivative (Eq. 1-3); G' = dt * grad u
+        {
+            const T gx = d1x[0], gy = d1y[0], ux = ctr[1], uy = ctr[2];
+            const T Gxx = d1x[1], Gxy = d1y[1], Gyx = d1x[2], Gyy = d1y[2], Gzx = d1x[3], Gzy = d1y[3];
+            const T Dh = Gxx + Gyy;
+            const T ug = fma_(uy, gy, ux * gx);
+            const T P0 = fma_(-c.dt, ug, -Dh);
+            const T h = fma_(-c.nu23, Dh, -c.cs2dt);
+            const T nsym = c.nu * (Gxy + Gyx);
+            const T kx = fma_(c.nu2, Gxx, h), ky = fma_(c.nu2, Gyy, h);
+            T tx = inpl[0], ty = inpl[1], tz = inpl[2];
+            tx = fma_(-ux, Gxx, tx);
+            ty = fma_(-ux, Gyx, ty);
+            tx = fma_(-uy, Gxy, tx);
+            ty = fma_(-uy, Gyy, ty);
+            tx = fma_(gx, kx, tx);
+            ty = fma_(gy, ky, ty);
+            tx = fma_(nsym, gy, tx);
+            ty = fma_(nsym, gx, ty);
+            tz = fma_(Gzx, fma_(c.nu, gx, -ux), tz);
+            tz = fma_(Gzy, fma_(c.nu, gy, -uy), tz);
+            const T pl[3] = {tx, ty, tz};
+            if (PATH55) {
+                const T* e[3] = {ex, ey, ez};
 #pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                st.lin[i][(n8 + 3) & 7] = -(c.mq[2] * e[i][2]);  // first contribution to output t+3
-                st.lin[i][(n8 + 2) & 7] -= c.mq[1] * e[i][1];
-                st.lin[i][(n8 + 1) & 7] -= c.mq[0] * e[i][0];
-                st.lin[i][n8] += inpl[i];
-                st.lin[i][(n8 + 7) & 7] += c.mq[0] * e[i][0];
-                st.lin[i][(n8 + 6) & 7] += c.mq[1] * e[i][1];
-                st.lin[i][(n8 + 5) & 7] += c.mq[2] * e[i][2];  // output t-3 is complete
+                for (int i = 0; i < 3; ++i) {
+                    st.lin[i][(n8 + 3) & 7] = -(c.mq[2] * e[i][2]);  // first contribution to output t+3
+                    st.lin[i][(n8 + 2) & 7] = fma_(-c.mq[1], e[i][1], st.lin[i][(n8 + 2) & 7]);
+                    st.lin[i][(n8 + 1) & 7] = fma_(-c.mq[0], e[i][0], st.lin[i][(n8 + 1) & 7]);
+                    st.lin[i][n8] += pl[i];
+                    st.lin[i][(n8 + 7) & 7] = fma_(c.mq[0], e[i][0], st.lin[i][(n8 + 7) & 7]);
+                    st.lin[i][(n8 + 6) & 7] = fma_(c.mq[1], e[i][1], st.lin[i][(n8 + 6) & 7]);
+                    st.lin[i][(n8 + 5) & 7] = fma_(c.mq[2], e[i][2], st.lin[i][(n8 + 5) & 7]);  // output t-3 is complete
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < 3; ++i) st.lin[i][n8] = pl[i];
             }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 3; ++i) st.lin[i][n8] = inpl[i];
+            st.dl[0][n4] = gx;
+            st.dl[1][n4] = gy;
+            st.dl[2][n4] = Gzx;
+            st.dl[3][n4] = Gzy;
+            st.dl[4][n4] = Dh;
+            st.dl[5][n4] = P0;
         }
         if (!out) return;
-        // ---- output plane z = t - 3: z derivatives from the window, Eq. 1-3, Eq. 10
+        // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
         constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
         T d1z[4], fc[4];
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
+            const T* a = f == 0 ? c.ar : c.au;
             fc[f] = st.win[f][cz];
-            d1z[f] = c.a[0] * (st.win[f][(cz + 1) & 7] - st.win[f][(cz + 7) & 7]) + c.a[1] * (st.win[f][(cz + 2) & 7] - st.win[f][(cz + 6) & 7]) +
-                     c.a[2] * (st.win[f][(cz + 3) & 7] - st.win[f][(cz + 5) & 7]);
+            d1z[f] = fma_(a[2], st.win[f][(cz + 3) & 7] - st.win[f][(cz + 5) & 7],
+                          fma_(a[1], st.win[f][(cz + 2) & 7] - st.win[f][(cz + 6) & 7], a[0] * (st.win[f][(cz + 1) & 7] - st.win[f][(cz + 7) & 7])));
         }
-        T lin[3];
+        T lz[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             const T* bz = i == 2 ? c.lq : c.lo;
             const int f = i + 1;
-            lin[i] = st.lin[i][cz] + (bz[0] * fc[f] + bz[1] * (st.win[f][(cz + 1) & 7] + st.win[f][(cz + 7) & 7]) +
-                                      bz[2] * (st.win[f][(cz + 2) & 7] + st.win[f][(cz + 6) & 7]) +
-                                      bz[3] * (st.win[f][(cz + 3) & 7] + st.win[f][(cz + 5) & 7]));
+            T v = fma_(bz[0], fc[f], st.lin[i][cz]);
+            v = fma_(bz[1], st.win[f][(cz + 1) & 7] + st.win[f][(cz + 7) & 7], v);
+            v = fma_(bz[2], st.win[f][(cz + 2) & 7] + st.win[f][(cz + 6) & 7], v);
+            v = fma_(bz[3], st.win[f][(cz + 3) & 7] + st.win[f][(cz + 5) & 7], v);
+            lz[i] = v;
         }
-        const T g[3] = {st.dl[0][r4], st.dl[1][r4], d1z[0]};
-        const T u[3] = {fc[1], fc[2], fc[3]};
-        T G[3][3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            G[i][0] = st.dl[2 * (i + 1)][r4];
-            G[i][1] = st.dl[2 * (i + 1) + 1][r4];
-            G[i][2] = d1z[i + 1];
-        }
-        const T div = G[0][0] + G[1][1] + G[2][2];
+        const T gxd = st.dl[0][r4], gyd = st.dl[1][r4], Gzxd = st.dl[2][r4], Gzyd = st.dl[3][r4], Dhd = st.dl[4][r4], P0d = st.dl[5][r4];
+        const T gz = d1z[0], Gxz = d1z[1], Gyz = d1z[2], Gzz = d1z[3], uz = fc[3];
+        const T divp = Dhd + Gzz;  // dt * div u
         T Rv[4];
-        Rv[0] = -(u[0] * g[0] + u[1] * g[1] + u[2] * g[2]) - div;
-        const T tdiv = c.nu23 * div;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            const T adv = u[0] * G[i][0] + u[1] * G[i][1] + u[2] * G[i][2];
-            const T sg = (G[i][0] + G[0][i]) * g[0] + (G[i][1] + G[1][i]) * g[1] + (G[i][2] + G[2][i]) * g[2];
-            Rv[1 + i] = (c.nu * sg - tdiv * g[i]) - adv - c.cs2 * g[i] + lin[i];
-        }
+        Rv[0] = fma_(-(c.dt * uz), gz, P0d - Gzz);
+        const T ngz = c.nu * gz, m23 = c.nu23 * Gzz;
+        T rx = lz[0], ry = lz[1], rz = lz[2];
+        rx = fma_(-uz, Gxz, rx);
+        ry = fma_(-uz, Gyz, ry);
+        rz = fma_(-uz, Gzz, rz);
+        rx = fma_(ngz, Gxz + Gzxd, rx);
+        ry = fma_(ngz, Gyz + Gzyd, ry);
+        rz = fma_(gz, fma_(c.nu2, Gzz, fma_(-c.nu23, divp, -c.cs2dt)), rz);
+        rx = fma_(-m23, gxd, rx);
+        ry = fma_(-m23, gyd, ry);
+        rz = fma_(c.nu * gxd, Gxz, rz);
+        rz = fma_(c.nu * gyd, Gyz, rz);
+        Rv[1] = rx;
+        Rv[2] = ry;
+        Rv[3] = rz;
         if (store_ok) {
-            if (!PATH55) *dv = div;
+            if (!PATH55) *dv = divp;
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
-                const T wn = s.read_w ? s.alpha * wold[f] + s.dt * Rv[f] : s.dt * Rv[f];
-                if (s.write_w) wq[f * n] = wn;
-                if (s.write_f) fo[f * fs] = fc[f] + s.beta * wn;
+                const T wn = c.read_w ? fma_(c.alpha, wold[f], Rv[f]) : Rv[f];
+                if (c.write_w) wq[f * n] = wn;
+                if (c.write_f) fo[f * fs] = fma_(c.beta, wn, fc[f]);
             }
         }
     }
 
     static __device__ __forceinline__ void run(const CUtensorMap* tm, T* __restrict__ Fout, T* __restrict__ W, T* __restrict__ Div,
-                                               const Geom& g, const TCoef<T>& c, const Sub<T>& s, int zc) {
+                                               const Geom& g, const KC<T>& c, int zc) {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
-        uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)S * STAGE * sizeof(T));
+        uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NS * STAGE * sizeof(T));
+        uint64_t* empty = full + NS;
         const int tx = threadIdx.x, ty = threadIdx.y;
         const int tid = ty * TX + tx;
         const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
         const int zs = blockIdx.z * zc, ze = min(zs + zc, g.nz);
         const int np = ze - zs + 2 * R;  // staged planes t = zs-3 .. ze+2
-        const int bx = g.gx + X0 - 4, by = g.gy + Y0 - R, bz = g.gz + zs - R;
+        // TMA box origin; the tensor map counts scalars along x, a value is `lanes` of them
+        const int bx = (g.gx + X0 - 4) * Scalar<T>::lanes, by = g.gy + Y0 - R, bz = g.gz + zs - R;
         constexpr uint32_t kStageBytes = (uint32_t)(STAGE * sizeof(T));
         if (tid == 0) {
 #pragma unroll
-            for (int i = 0; i < S; ++i) mbar_init(&full[i], 1);
+            for (int i = 0; i < NS; ++i) {
+                mbar_init(&full[i], 1);
+                mbar_init(&empty[i], WARPS);
+            }
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         __syncthreads();
         if (tid == 0) {
-            for (int i = 0; i < S && i < np; ++i) {
+            for (int i = 0; i < NS && i < np; ++i) {
                 mbar_expect_tx(&full[i], kStageBytes);
                 tma_load_4d(sm + i * STAGE, tm, &full[i], bx, by, bz + i, 0);
             }
@@ -232,7 +289,7 @@ struct Tiled {
             for (int q = 0; q < 3; ++q) st.lin[q][a] = T(0);
         }
 #pragma unroll
-        for (int q = 0; q < 8; ++q)
+        for (int q = 0; q < 6; ++q)
 #pragma unroll
             for (int a = 0; a < 4; ++a) st.dl[q][a] = T(0);
 
@@ -241,25 +298,30 @@ struct Tiled {
             for (int ph = 0; ph < 8; ++ph) {
                 const int p = pb + ph;
                 if (p < np) {
-                    mbar_wait(&full[ph & 3], (uint32_t)((p >> 2) & 1));
+                    mbar_wait(&full[ph], (uint32_t)((p >> 3) & 1));
                     switch (ph) {  // ph is a compile-time constant after unrolling
-                        case 0: step<0>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 1: step<1>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 2: step<2>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 3: step<3>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 4: step<4>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 5: step<5>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        case 6: step<6>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
-                        default: step<7>(st, sp0, c, s, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 0: step<0>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 1: step<1>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 2: step<2>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 3: step<3>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 4: step<4>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 5: step<5>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        case 6: step<6>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
+                        default: step<7>(st, sp0, c, p, store_ok, W + ow, W + ow, Fout + of, Div + of, g.fs, g.n); break;
                     }
                     if (p >= 2 * R && store_ok) {
                         ow += plane_w;
                         of += plane_f;
                     }
-                    __syncthreads();  // every thread is done reading stage ph&3
-                    if (tid == 0 && p + S < np) {
-                        mbar_expect_tx(&full[ph & 3], kStageBytes);
-                        tma_load_4d(sm + (ph & 3) * STAGE, tm, &full[ph & 3], bx, by, bz + p + S, 0);
+                    // this warp is done reading stage ph: hand it back; thread 0 refills the stage every warp has
+                    // released one plane earlier, so it never waits for a warp that is less than a plane behind
+                    __syncwarp();
+                    if ((tid & 31) == 0) mbar_arrive(&empty[ph]);
+                    if (tid == 0 && p >= 1 && p - 1 + NS < np) {
+                        const int sprev = (ph + 7) & 7;
+                        mbar_wait(&empty[sprev], (uint32_t)(((p - 1) >> 3) & 1));
+                        mbar_expect_tx(&full[sprev], kStageBytes);
+                        tma_load_4d(sm + sprev * STAGE, tm, &full[sprev], bx, by, bz + p - 1 + NS, 0);
                     }
                 }
             }
@@ -270,11 +332,11 @@ struct Tiled {
 template <class T, bool PATH55, int TX, int TY>
 __global__ void __launch_bounds__(TX* TY, 1)
     k_tiled_main(const __grid_constant__ CUtensorMap tm, T* __restrict__ Fout, T* __restrict__ W, T* __restrict__ Div, const Geom g,
-                 const TCoef<T> c, const Sub<T> s, int zc) {
-    Tiled<T, PATH55, TX, TY>::run(&tm, Fout, W, Div, g, c, s, zc);
+                 const __grid_constant__ KC<T> c, int zc) {
+    Tiled<T, PATH55, TX, TY>::run(&tm, Fout, W, Div, g, c, zc);
 }
 
-// Tile shape per element type (registers per thread bound the CTA size).
+// Tile shape per value type (registers per thread bound the CTA size).
 template <class T>
 struct TileShape;
 template <>
@@ -283,6 +345,10 @@ struct TileShape<float> {
 };
 template <>
 struct TileShape<double> {
+    static constexpr int TX = 32, TY = 8;
+};
+template <>
+struct TileShape<V2> {
     static constexpr int TX = 32, TY = 8;
 };
 
@@ -299,7 +365,7 @@ struct TiledState {
     char err[256] = "";
 };
 
-inline bool tiled_supported(const Geom& g, int /*dtype*/) { return g.nx >= 8 && g.ny >= 8 && g.nz >= 8; }
+inline bool tiled_supported(const Geom& g) { return g.nx >= 4 && g.ny >= 4 && g.nz >= 4; }
 
 inline PFN_encodeTiled tiled_encode_fn() {
     static PFN_encodeTiled fn = nullptr;
@@ -315,19 +381,22 @@ inline PFN_encodeTiled tiled_encode_fn() {
     return fn;
 }
 
+// Tensor map of one copy of the four padded fields: dims (x in scalars, y, z, field), box = one staged plane.
 template <class T>
 static int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, const Geom& g) {
+    typedef typename Scalar<T>::type S;
+    constexpr int L = Scalar<T>::lanes;
     PFN_encodeTiled enc = tiled_encode_fn();
     if (!enc) {
         snprintf(ts.err, sizeof(ts.err), "cuTensorMapEncodeTiled is not available from this driver");
         return 3;
     }
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
-    const cuuint64_t dims[4] = {(cuuint64_t)g.px, (cuuint64_t)g.py, (cuuint64_t)g.pz, 4};
+    const cuuint64_t dims[4] = {(cuuint64_t)g.px * L, (cuuint64_t)g.py, (cuuint64_t)g.pz, 4};
     const cuuint64_t strides[3] = {(cuuint64_t)g.px * sizeof(T), (cuuint64_t)g.px * g.py * sizeof(T), (cuuint64_t)g.fs * sizeof(T)};
-    const cuuint32_t box[4] = {(cuuint32_t)(TX + 8), (cuuint32_t)(TY + 2 * R), 1, 4};
+    const cuuint32_t box[4] = {(cuuint32_t)((TX + 8) * L), (cuuint32_t)(TY + 2 * R), 1, 4};
     const cuuint32_t estr[4] = {1, 1, 1, 1};
-    CUresult r = enc(tm, sizeof(T) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box,
+    CUresult r = enc(tm, sizeof(S) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box,
                      estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                      CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -338,7 +407,8 @@ static int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, const Geo
 }
 
 template <class T>
-static int tiled_prepare_t(TiledState& ts, const Geom& g, void* F0, void* F1) {
+static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1) {
+    ts.ready = false;
     int rc = tiled_make_map<T>(ts, &ts.tmF[0], F0, g);
     if (rc == 0) rc = tiled_make_map<T>(ts, &ts.tmF[1], F1, g);
     if (rc) return rc;
@@ -358,11 +428,11 @@ static int tiled_prepare_t(TiledState& ts, const Geom& g, void* F0, void* F1) {
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
     // z chunking: one CTA per SM is resident; pick the number of chunks that fills whole waves of SMs best while
-    // keeping the 6-plane warm-up of every chunk below ~5 %.
+    // keeping the 6-plane warm-up of every chunk small.
     const long long tiles = (long long)((g.nx + TX - 1) / TX) * ((g.ny + TY - 1) / TY);
     int best_c = 1;
     double best_cost = 1e300;
-    for (int cks = 1; cks <= g.nz / 8 && cks <= 64; ++cks) {
+    for (int cks = 1; cks <= (g.nz + 7) / 8 && cks <= 64; ++cks) {
         const int zc = (g.nz + cks - 1) / cks;
         const int real = (g.nz + zc - 1) / zc;
         const long long ctas = tiles * real;
@@ -379,48 +449,54 @@ static int tiled_prepare_t(TiledState& ts, const Geom& g, void* F0, void* F1) {
 }
 
 inline const char* tiled_error_of(const TiledState& ts) { return ts.err; }
-
-inline int tiled_prepare(TiledState& ts, const Geom& g, int dtype, void* F0, void* F1, void* /*Div*/) {
-    ts.ready = false;
-    return dtype == 0 ? tiled_prepare_t<float>(ts, g, F0, F1) : tiled_prepare_t<double>(ts, g, F0, F1);
-}
 inline void tiled_release(TiledState& ts) { ts.ready = false; }
 
 template <class T>
-static TCoef<T> make_tcoef(double dx, double nu, double cs, bool path55) {
+static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, double alpha, double beta, int read_w, int write_f,
+                     int write_w) {
+    typedef typename Scalar<T>::type S;
     const double dx2 = dx * dx;
     const double b[4] = {-490.0 / (180.0 * dx2), 270.0 / (180.0 * dx2), -27.0 / (180.0 * dx2), 2.0 / (180.0 * dx2)};
     const double cm[3] = {270.0 / (720.0 * dx2), -27.0 / (720.0 * dx2), 2.0 / (720.0 * dx2)};
+    const double a[3] = {45.0 / (60.0 * dx), -9.0 / (60.0 * dx), 1.0 / (60.0 * dx)};
     const double own = path55 ? 4.0 * nu / 3.0 : nu;
-    TCoef<T> k;
-    k.a[0] = T(45.0 / (60.0 * dx));
-    k.a[1] = T(-9.0 / (60.0 * dx));
-    k.a[2] = T(1.0 / (60.0 * dx));
-    for (int m = 0; m < 4; ++m) {
-        k.lo[m] = T(nu * b[m]);
-        k.lq[m] = T(own * b[m]);
+    KC<T> k;
+    for (int m = 0; m < 3; ++m) {
+        k.ar[m] = T(S(a[m]));
+        k.au[m] = T(S(dt * a[m]));
+        k.mq[m] = T(S(dt * nu / 3.0 * cm[m]));
     }
-    k.cxy[0] = T((own + nu) * b[0]);
-    k.cxy[1] = T((own + nu) * b[0]);
-    k.cxy[2] = T(2.0 * nu * b[0]);
-    for (int m = 0; m < 3; ++m) k.mq[m] = T(nu / 3.0 * cm[m]);
-    k.nu = T(nu);
-    k.cs2 = T(cs * cs);
-    k.nu23 = T(2.0 * nu / 3.0);
+    for (int m = 0; m < 4; ++m) {
+        k.lo[m] = T(S(dt * nu * b[m]));
+        k.lq[m] = T(S(dt * own * b[m]));
+    }
+    k.cxy[0] = T(S(dt * (own + nu) * b[0]));
+    k.cxy[1] = T(S(dt * (own + nu) * b[0]));
+    k.cxy[2] = T(S(dt * 2.0 * nu * b[0]));
+    k.nu = T(S(nu));
+    k.nu2 = T(S(2.0 * nu));
+    k.nu23 = T(S(2.0 * nu / 3.0));
+    k.cs2dt = T(S(cs * cs * dt));
+    k.dt = T(S(dt));
+    k.alpha = T(S(alpha));
+    k.beta = T(S(beta));
+    k.read_w = read_w;
+    k.write_f = write_f;
+    k.write_w = write_w;
     return k;
 }
 
-// Launch of the main kernel of one substep (fused 55-point kernel, or pass 1 of the 19-point path).
+// Launch of the main kernel of one substep (fused 55-point kernel, or pass 1 of the 19-point path, which
+// leaves dt * div u in Div).
 template <class T>
-static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, double dx, double nu, double cs,
-                             const Sub<T>& s, cudaStream_t stream) {
+static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
+                             cudaStream_t stream) {
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
     dim3 block(TX, TY, 1), grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + ts.zc - 1) / ts.zc);
-    const TCoef<T> c = make_tcoef<T>(dx, nu, cs, path55 != 0);
     if (path55)
-        k_tiled_main<T, true, TX, TY><<<grid, block, Tiled<T, true, TX, TY>::SMEM, stream>>>(ts.tmF[cur], Fout, W, Div, g, c, s, ts.zc);
+        k_tiled_main<T, true, TX, TY><<<grid, block, Tiled<T, true, TX, TY>::SMEM, stream>>>(ts.tmF[cur], Fout, W, Div, g, c, ts.zc);
     else
-        k_tiled_main<T, false, TX, TY><<<grid, block, Tiled<T, false, TX, TY>::SMEM, stream>>>(ts.tmF[cur], Fout, W, Div, g, c, s, ts.zc);
+        k_tiled_main<T, false, TX, TY><<<grid, block, Tiled<T, false, TX, TY>::SMEM, stream>>>(ts.tmF[cur], Fout, W, Div, g, c, ts.zc);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 

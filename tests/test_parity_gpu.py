@@ -31,7 +31,7 @@ def relinf(A, B):
 
 
 def variants(fd6):
-    return [fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_TILED]
+    return [fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_TILED, fd6.FD_VARIANT_PAIRED]
 
 
 def make_ctx(fd6, shape_xyz, dx, nu, cs, dtype, path, variant):
@@ -89,7 +89,7 @@ def test_load_store_round_trip_is_bit_exact(mods, dtype, where):
 
 # ------------------------------------------------------------ config C1: full grid, both paths
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_c1_one_step_and_rhs_full_grid_fp64(mods, path, variant):
     O, fd6, I = mods
     cfg = I.CONFIGS["C1"]
@@ -111,7 +111,7 @@ def test_c1_one_step_and_rhs_full_grid_fp64(mods, path, variant):
 @pytest.mark.parametrize("shape", [(40, 13, 9), (8, 8, 8), (132, 70, 20), (72, 33, 41)])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_ragged_grids_three_steps(mods, shape, dtype, path, variant):
     O, fd6, I = mods
     rng = np.random.default_rng(shape[0] * 1000 + shape[1] * 10 + path)
@@ -134,7 +134,7 @@ def test_ragged_grids_three_steps(mods, shape, dtype, path, variant):
 
 # --------------------------------------- config C2 (128^3 fp32): one step, full grid, both paths
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_c2_one_step_full_grid_fp32(mods, path, variant):
     O, fd6, I = mods
     cfg = I.CONFIGS["C2"]
@@ -152,7 +152,7 @@ def test_c2_one_step_full_grid_fp32(mods, path, variant):
 # ----------------------------------------------------------- degenerate and invariant cases
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_uniform_state_at_rest_is_a_fixed_point(mods, dtype, path, variant):
     O, fd6, I = mods
     shape = (32, 16, 24)
@@ -170,7 +170,7 @@ def test_uniform_state_at_rest_is_a_fixed_point(mods, dtype, path, variant):
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_periodic_shift_equivariance_is_bitwise(mods, dtype, path, variant):
     """step(roll(F)) == roll(step(F)) bit for bit: no cell's arithmetic may depend on its position in a tile."""
     O, fd6, I = mods
@@ -189,7 +189,7 @@ def test_periodic_shift_equivariance_is_bitwise(mods, dtype, path, variant):
 
 
 @pytest.mark.parametrize("path", [0, 1])
-@pytest.mark.parametrize("variant", [1, 2])
+@pytest.mark.parametrize("variant", [1, 2, 3])
 def test_shear_mode_decay_closed_form_on_gpu(mods, path, variant):
     """P6 on the GPU: the discrete twin of the paper's Eq. 22 test."""
     O, fd6, I = mods
@@ -316,4 +316,55 @@ def test_profile_counters_count_the_launches(mods):
     assert n == 6 and ms > 0
     total = sum(ctx.fd_get_profile(k)[1] for k in range(fd6.FD_K_COUNT))
     assert total == ctx.fd_kernel_launches() - before
+    ctx.fd_destroy()
+
+
+# ------------------------------------------------- layout conversion when the variant changes
+def test_variant_switch_carries_a_loaded_state_across_layouts(mods):
+    """PAIRED stores cells k and k+nz/2 side by side; switching variants converts the resident state.  Every
+    variant, entered from either layout, must continue the same trajectory (each compared with the oracle)."""
+    O, fd6, I = mods
+    shape = (40, 24, 18)
+    rng = np.random.default_rng(77)
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.1, "f32")
+    ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32)
+    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED  # AUTO: fp32, even nz
+    ctx.load_state(F)
+    order = [fd6.FD_VARIANT_TILED, fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_PAIRED, fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_TILED]
+    for n, v in enumerate(order, start=1):
+        ctx.fd_set_variant(v)
+        assert ctx.fd_get_info().variant == v
+        assert np.array_equal(ctx.store_state(), F) or n > 1  # the conversion itself is exact
+        ctx.fd_rk3_step(dt, 1)
+        got = ctx.store_state()
+        ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, n, 0)
+        assert relinf(got, ref) <= n * TOL["f32"]
+    # fd_rhs through the paired layout, host and device destinations agree with the oracle
+    ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)
+    ctx.load_state(F)
+    R = ctx.rhs_state()
+    assert relinf(R, O.rhs(F.astype(np.float64), dx, nu, cs, 0)) <= TOL["f32"]
+    assert np.array_equal(ctx.store_state(), F)
+    import torch
+    Rd = torch.empty((4,) + shape[::-1], dtype=torch.float32, device="cuda")
+    ctx.rhs_state(Rd)
+    ctx.fd_sync()
+    assert np.array_equal(Rd.cpu().numpy(), R)
+    ctx.fd_destroy()
+
+
+def test_paired_variant_is_refused_where_it_cannot_run(mods):
+    O, fd6, I = mods
+    ctx = fd6.Fd(16, 16, 9, 0.1, 0.01, 1.0, fd6.FD_F32)   # odd nz
+    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_TILED
+    with pytest.raises(fd6.FdError) as e:
+        ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)
+    assert e.value.code == fd6.FD_EUNSUPPORTED
+    ctx.fd_destroy()
+    ctx = fd6.Fd(16, 16, 16, 0.1, 0.01, 1.0, fd6.FD_F64)  # fp64
+    with pytest.raises(fd6.FdError) as e:
+        ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)
+    assert e.value.code == fd6.FD_EUNSUPPORTED
     ctx.fd_destroy()
