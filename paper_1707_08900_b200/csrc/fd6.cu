@@ -276,7 +276,7 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
         if (tiled) {
             const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w);
-            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, c->stream))
+            if (tiled_launch_main<T>(c->tiled, p55, c->cur, g, kc, c->stream))
                 return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (p55) {
             k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
@@ -461,7 +461,7 @@ static int resolve_variant(fd_ctx* c) {
     if (want == FD_VARIANT_TILED) rc = set_layout(c, false);
     if (rc) return rc;
     if (want == FD_VARIANT_TILED || want == FD_VARIANT_PAIRED) {
-        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1])) : 4;
+        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W, c->Div)) : 4;
         if (rc != FD_OK) {
             if (c->variant_req == FD_VARIANT_AUTO) {
                 want = FD_VARIANT_DIRECT;
@@ -570,6 +570,8 @@ extern "C" int fd_set_path(fd_ctx* c, int path) {
         int rc = ctx_alloc(c, &c->Div, c->div_bytes);
         if (rc) return rc;
         FD_CUDA(cudaMemsetAsync(c->Div, 0, c->div_bytes, c->stream));
+        rc = resolve_variant(c);  // the tiled kernels store div u through a tensor map of the new array
+        if (rc) return rc;
     }
     c->path = path;
     return FD_OK;
