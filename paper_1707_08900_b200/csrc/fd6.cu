@@ -276,7 +276,7 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
         if (tiled) {
             const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w);
-            if (tiled_launch_main<T>(c->tiled, p55, c->cur, g, kc, c->stream))
+            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, c->stream))
                 return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (p55) {
             k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
@@ -408,19 +408,20 @@ static int do_rhs(fd_ctx* c, void* const out[4], int where) {
     int rc = launch_substep<T>(c, sub);
     if (rc) return rc;
     const size_t nscal = (size_t)c->nx * c->ny * c->nz;
-    if (Scalar<T>::lanes == 1) {  // the w arrays already are in the caller's layout
+    if constexpr (Scalar<T>::lanes == 1) {  // the w arrays already are in the caller's layout
         for (int q = 0; q < 4; ++q)
             FD_CUDA(cudaMemcpyAsync(out[q], (const S*)c->W + (size_t)q * nscal, nscal * sizeof(S),
                                     where == FD_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
         if (where == FD_HOST) FD_CUDA(cudaStreamSynchronize(c->stream));
         return FD_OK;
+    } else {
+        // paired layout: un-pair w; the write copy of the fields is free scratch for the host staging
+        S* dst[4];
+        for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (S*)c->F[1 - c->cur] + (size_t)q * nscal : (S*)out[q];
+        rc = do_unpack<T>(c, (const T*)c->W, dense_geom(c->g), dst);
+        if (rc) return rc;
+        return where == FD_HOST ? copy_out<S>(c, (const S*)c->F[1 - c->cur], out) : FD_OK;
     }
-    // paired layout: un-pair w; the write copy of the fields is free scratch for the host staging
-    S* dst[4];
-    for (int q = 0; q < 4; ++q) dst[q] = where == FD_HOST ? (S*)c->F[1 - c->cur] + (size_t)q * nscal : (S*)out[q];
-    rc = do_unpack<T>(c, (const T*)c->W, dense_geom(c->g), dst);
-    if (rc) return rc;
-    return where == FD_HOST ? copy_out<S>(c, (const S*)c->F[1 - c->cur], out) : FD_OK;
 }
 
 // Switch between the plain and the paired layout, carrying a loaded state across through the w scratch.
@@ -461,7 +462,7 @@ static int resolve_variant(fd_ctx* c) {
     if (want == FD_VARIANT_TILED) rc = set_layout(c, false);
     if (rc) return rc;
     if (want == FD_VARIANT_TILED || want == FD_VARIANT_PAIRED) {
-        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W, c->Div)) : 4;
+        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W)) : 4;
         if (rc != FD_OK) {
             if (c->variant_req == FD_VARIANT_AUTO) {
                 want = FD_VARIANT_DIRECT;
@@ -570,8 +571,6 @@ extern "C" int fd_set_path(fd_ctx* c, int path) {
         int rc = ctx_alloc(c, &c->Div, c->div_bytes);
         if (rc) return rc;
         FD_CUDA(cudaMemsetAsync(c->Div, 0, c->div_bytes, c->stream));
-        rc = resolve_variant(c);  // the tiled kernels store div u through a tensor map of the new array
-        if (rc) return rc;
     }
     c->path = path;
     return FD_OK;

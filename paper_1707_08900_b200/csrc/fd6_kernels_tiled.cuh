@@ -2,16 +2,15 @@
 // (DESIGN.md "Kernels").  One template, three value types: float, double, and V2 (two fp32 cells per value,
 // packed FFMA2/FADD2/FMUL2 arithmetic — the paired layout).
 //
-// One CTA owns a TX x TY column of values and marches along z through a chunk of planes.  All global traffic
-// goes through the TMA unit; no thread ever forms a global address:
-//   in   plane t of the four fields + radius-3 halo: ONE 4-D box copy (cp.async.bulk.tensor, mbarrier
+// One CTA owns a TX x TY column of values and marches along z through a chunk of planes.
+//   in   plane t of the four fields + radius-3 halo: ONE 4-D TMA box copy (cp.async.bulk.tensor, mbarrier
 //        complete_tx) into an NS-deep ring of stages; the w values of the output plane: one more box copy into
-//        a 4-deep ring (only on substeps that read w).  A stage is handed back to the producer thread through
-//        an "empty" mbarrier on which every warp arrives once it is done with the plane, so there is no CTA-wide
-//        barrier in the loop.
-//   out  every warp writes its 32 new F and w values per field into a double-buffered staging row and lane 0
-//        sends it with one TMA box store per tensor (cp.async.bulk.tensor ... bulk_group); the tensor maps clip
-//        ragged tiles.
+//        a 4-deep ring (only on substeps that read w), so no thread waits on a global load.  A stage is handed
+//        back to the producer thread through an "empty" mbarrier on which every warp arrives once it is done
+//        with the plane, so there is no CTA-wide barrier in the loop.
+//   out  F_out, w (and div u) go straight from registers to global memory: a warp writes one 256-byte row
+//        segment per array.  (Staging them in shared memory for TMA box stores was measured 5-11 % slower: the
+//        kernel is bound by shared-memory bandwidth.)
 // Each thread owns one column and keeps everything that couples planes in registers:
 //   win[f][8]   sliding window of its own column along z                     -> D1z, D2z          (Eq. 6, 7)
 //   lin[i][8]   accumulator ring of everything of dt*rhs_i that is known when a plane is staged: the in-plane
@@ -49,25 +48,24 @@ struct KC {
 
 // The tensor maps of one launch (each 128 bytes, passed by value as a __grid_constant__ parameter).
 struct Maps {
-    CUtensorMap f_in;    // padded fields, read copy:  box (TX+8, TY+6, 1, 4)
-    CUtensorMap f_out;   // padded fields, write copy: box (32, 1, 1, 4), x clipped at the end of the interior
-    CUtensorMap w_ld;    // dense w:                   box (TX, TY, 1, 4)
-    CUtensorMap w_st;    // dense w:                   box (32, 1, 1, 4)
-    CUtensorMap div_st;  // padded div u (19-point):   box (32, 1, 1, 1)
+    CUtensorMap f_in;  // padded fields, read copy: box (TX+8, TY+6, 1, 4)
+    CUtensorMap w_ld;  // dense w:                  box (TX, TY, 1, 4)
 };
 
 // ---- mbarrier / TMA primitives (PTX ISA: mbarrier, cp.async.bulk.tensor) --------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t* b, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
+// All helpers take 32-bit shared-window addresses, formed once per kernel from the base of the dynamic
+// shared memory, so that the plane loop holds no generic-to-shared conversions.
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
 }
-__device__ __forceinline__ void mbar_expect_tx(uint64_t* b, uint32_t bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint64_t* b) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
@@ -76,31 +74,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t* b, uint32_t parity) {
         "@p bra DONE_%=;\n"
         "bra WAIT_%=;\n"
         "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(b)),
+        "}\n" ::"r"(bar),
         "r"(parity)
         : "memory");
 }
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, uint64_t* bar, int c0, int c1, int c2, int c3) {
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm, uint32_t bar, int c0, int c1, int c2, int c3) {
     asm volatile(
-        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(
-            smem_u32(dst)),
-        "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+        "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(dst),
+        "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
-__device__ __forceinline__ void tma_store_4d(const void* src, const CUtensorMap* tm, int c0, int c1, int c2, int c3) {
-    asm volatile("cp.async.bulk.tensor.4d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];" ::"l"(tm),
-                 "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
-                 : "memory");
-}
-__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
-// wait until at most N of this thread's bulk groups still READ their shared-memory source
-template <int N>
-__device__ __forceinline__ void bulk_wait_read() {
-    asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
-}
-// make this thread's shared-memory writes visible to the async (TMA) proxy
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-
 template <class T, bool PATH55, int TX, int TY>
 struct Tiled {
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
@@ -113,13 +96,8 @@ struct Tiled {
     static constexpr int WSTAGE = 4 * WFIELD;
     static constexpr int THREADS = TX * TY;
     static constexpr int WARPS = THREADS / 32;
-    static constexpr int WPR = TX / 32;                // warps per tile row
-    static constexpr int NSLOT = PATH55 ? 8 : 9;       // staging rows of a warp: 4 F_out, 4 w, (dt div u)
-    static constexpr int OBUF = NSLOT * 32;            // values per warp and staging buffer
-    static constexpr int OUT = 2 * WARPS * OBUF;       // double-buffered
-    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE + OUT) * sizeof(T) + (2 * NS + NW) * sizeof(uint64_t);
-    static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0 && (OBUF * sizeof(T)) % 128 == 0,
-                  "TMA shared-memory boxes must stay 128-byte aligned");
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW) * sizeof(uint64_t);
+    static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
     struct State {
         T win[4][8];
@@ -128,10 +106,12 @@ struct Tiled {
     };
 
     // One plane.  sp0: this thread's centre in stage 0 of the F ring; wsp0: its element in stage 0 of the w ring;
-    // ob0: its lane's element in staging buffer 0 of its warp.  `out`: plane z = t - 3 is produced.
+    // gF, gW, gD: its cell of output plane z = t - 3 in F_out, w and div (field strides fs, n); `out`: that plane
+    // is produced; store_ok: the thread's column lies inside the grid.
     template <int PH>
-    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const T* __restrict__ wsp0, T* __restrict__ ob0,
-                                                const KC<T>& c, bool out, bool lane0) {
+    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const T* __restrict__ wsp0, const KC<T>& c,
+                                                bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
+                                                long long n, bool store_ok) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
         const T* sp = sp0 + n8 * STAGE;
         // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8)
@@ -264,33 +244,30 @@ struct Tiled {
         Rv[1] = rx;
         Rv[2] = ry;
         Rv[3] = rz;
-        // ---- Eq. 10 into the staging rows of this warp (the TMA store that last read this buffer has finished)
+        // ---- Eq. 10; coalesced 64/128/256-byte row segments per warp straight to global memory
         const T* wsp = wsp0 + ((PH + 2) & 3) * WSTAGE;  // w ring slot of plane index p - 6
-        T* ob = ob0 + (PH & 1) * (WARPS * OBUF);
-        if (lane0) bulk_wait_read<1>();
-        __syncwarp();
+        if (store_ok) {
 #pragma unroll
-        for (int f = 0; f < 4; ++f) {
-            const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD], Rv[f]) : Rv[f];
-            ob[(4 + f) * 32] = wn;
-            ob[f * 32] = fma_(c.beta, wn, fc[f]);
+            for (int f = 0; f < 4; ++f) {
+                const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD], Rv[f]) : Rv[f];
+                if (c.write_w) gW[f * n] = wn;
+                if (c.write_f) gF[f * fs] = fma_(c.beta, wn, fc[f]);
+            }
+            if (!PATH55) *gD = divp;
         }
-        if (!PATH55) ob[8 * 32] = divp;
-        fence_async_smem();
     }
 
-    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, int zc) {
+    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, int zc, T* __restrict__ Fout,
+                                               T* __restrict__ W, T* __restrict__ Div) {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
         T* smw = sm + NS * STAGE;
-        T* smo = smw + NW * WSTAGE;
-        uint64_t* full = reinterpret_cast<uint64_t*>(smo + OUT);
-        uint64_t* empty = full + NS;
-        uint64_t* wfull = empty + NS;
+        const uint32_t a_sm = smem_u32(smem_raw);
+        const uint32_t a_smw = a_sm + (uint32_t)(NS * STAGE * sizeof(T));
+        const uint32_t a_full = a_smw + (uint32_t)(NW * WSTAGE * sizeof(T)), a_empty = a_full + 8 * NS, a_wfull = a_empty + 8 * NS;
         const int tx = threadIdx.x, ty = threadIdx.y;
         const int tid = ty * TX + tx;
-        const int warp = tid >> 5, lane = tid & 31;
-        const bool lane0 = lane == 0, producer = tid == 0;
+        const bool lane0 = (tid & 31) == 0, producer = tid == 0;
         const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
         const int zs = blockIdx.z * zc, ze = min(zs + zc, g.nz);
         const int np = ze - zs + 2 * R;  // staged planes t = zs-3 .. ze+2
@@ -302,27 +279,29 @@ struct Tiled {
         if (producer) {
 #pragma unroll
             for (int i = 0; i < NS; ++i) {
-                mbar_init(&full[i], 1);
-                mbar_init(&empty[i], WARPS);
+                mbar_init(a_full + 8 * i, 1);
+                mbar_init(a_empty + 8 * i, WARPS);
             }
 #pragma unroll
-            for (int i = 0; i < NW; ++i) mbar_init(&wfull[i], 1);
+            for (int i = 0; i < NW; ++i) mbar_init(a_wfull + 8 * i, 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         __syncthreads();
         if (producer) {
             for (int i = 0; i < NS && i < np; ++i) {
-                mbar_expect_tx(&full[i], kStageBytes);
-                tma_load_4d(sm + i * STAGE, &m.f_in, &full[i], bx, by, bz + i, 0);
+                mbar_expect_tx(a_full + 8 * i, kStageBytes);
+                tma_load_4d(a_sm + i * kStageBytes, &m.f_in, a_full + 8 * i, bx, by, bz + i, 0);
             }
         }
-        // store coordinates of this warp's row (warp-uniform)
-        const int wy = warp / WPR, wx = (warp % WPR) * 32;
-        const bool row_ok = Y0 + wy < g.ny && X0 + wx < g.nx;
-        const int sxw = (X0 + wx) * L, sxf = (g.gx + X0 + wx) * L, syw = Y0 + wy, syf = g.gy + Y0 + wy;
         const T* sp0 = sm + (ty + R) * PXS + (tx + 4);
         const T* wsp0 = smw + ty * TX + tx;
-        T* ob0 = smo + warp * OBUF + lane;
+        // this thread's cell of output plane zs in the dense (w) and padded (F, div) arrays; advanced plane by plane
+        const int ci = X0 + tx, cj = Y0 + ty;
+        const bool store_ok = ci < g.nx && cj < g.ny;
+        const long long plane_w = (long long)g.nx * g.ny, plane_f = (long long)g.px * g.py;
+        long long ow = ci + (long long)g.nx * (cj + (long long)g.ny * zs);
+        long long of = (ci + g.gx) + (long long)g.px * ((cj + g.gy) + (long long)g.py * (zs + g.gz));
+        if (!store_ok) { ow = 0; of = 0; }
         State st;
 #pragma unroll
         for (int a = 0; a < 8; ++a) {
@@ -342,32 +321,26 @@ struct Tiled {
                 const int p = pb + ph;
                 if (p < np) {
                     const bool out = p >= 2 * R;  // planes 0..5 of a chunk only warm the window and the rings up
-                    mbar_wait(&full[ph], (uint32_t)((p >> 3) & 1));
-                    if (out && c.read_w) mbar_wait(&wfull[(ph + 2) & 3], (uint32_t)(((p - 2 * R) >> 2) & 1));
+                    mbar_wait(a_full + 8 * ph, (uint32_t)((p >> 3) & 1));
+                    if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
+#define FD6_STEP(K) step<K>(st, sp0, wsp0, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, store_ok)
                     switch (ph) {  // ph is a compile-time constant after unrolling
-                        case 0: step<0>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 1: step<1>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 2: step<2>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 3: step<3>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 4: step<4>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 5: step<5>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        case 6: step<6>(st, sp0, wsp0, ob0, c, out, lane0); break;
-                        default: step<7>(st, sp0, wsp0, ob0, c, out, lane0); break;
+                        case 0: FD6_STEP(0); break;
+                        case 1: FD6_STEP(1); break;
+                        case 2: FD6_STEP(2); break;
+                        case 3: FD6_STEP(3); break;
+                        case 4: FD6_STEP(4); break;
+                        case 5: FD6_STEP(5); break;
+                        case 6: FD6_STEP(6); break;
+                        default: FD6_STEP(7); break;
                     }
-                    // every lane has written its staging row and fenced it for the async proxy; this warp is also done
-                    // reading stage ph (F) and its w slot
+                    if (out && store_ok) {
+                        ow += plane_w;
+                        of += plane_f;
+                    }
+                    // this warp is done reading stage ph (F) and its w slot: hand them back
                     __syncwarp();
-                    if (lane0) {
-                        if (out && row_ok) {
-                            const T* src = smo + (ph & 1) * (WARPS * OBUF) + warp * OBUF;
-                            const int z = zs + p - 2 * R;
-                            if (c.write_f) tma_store_4d(src, &m.f_out, sxf, syf, g.gz + z, 0);
-                            if (c.write_w) tma_store_4d(src + 4 * 32, &m.w_st, sxw, syw, z, 0);
-                            if (!PATH55) tma_store_4d(src + 8 * 32, &m.div_st, sxf, syf, g.gz + z, 0);
-                            bulk_commit();
-                        }
-                        mbar_arrive(&empty[ph]);
-                    }
+                    if (lane0) mbar_arrive(a_empty + 8 * ph);
                     // thread 0 refills the stage every warp has released one plane earlier, so it never waits for a
                     // warp that is less than a plane behind; the w values of step q = p + 3 go into the slot step p - 1 used
                     if (producer && p >= 1) {
@@ -375,28 +348,29 @@ struct Tiled {
                         const bool more_f = p - 1 + NS < np;
                         const int q = p + 3;
                         const bool more_w = c.read_w && q >= 2 * R && q < np;
-                        if (more_f || more_w) mbar_wait(&empty[sprev], (uint32_t)(((p - 1) >> 3) & 1));
+                        if (more_f || more_w) mbar_wait(a_empty + 8 * sprev, (uint32_t)(((p - 1) >> 3) & 1));
                         if (more_f) {
-                            mbar_expect_tx(&full[sprev], kStageBytes);
-                            tma_load_4d(sm + sprev * STAGE, &m.f_in, &full[sprev], bx, by, bz + p - 1 + NS, 0);
+                            mbar_expect_tx(a_full + 8 * sprev, kStageBytes);
+                            tma_load_4d(a_sm + sprev * kStageBytes, &m.f_in, a_full + 8 * sprev, bx, by, bz + p - 1 + NS, 0);
                         }
                         if (more_w) {
                             const int ws = (ph + 5) & 3;  // (q - 6) & 3
-                            mbar_expect_tx(&wfull[ws], kWBytes);
-                            tma_load_4d(smw + ws * WSTAGE, &m.w_ld, &wfull[ws], X0 * L, Y0, zs + q - 2 * R, 0);
+                            mbar_expect_tx(a_wfull + 8 * ws, kWBytes);
+                            tma_load_4d(a_smw + ws * kWBytes, &m.w_ld, a_wfull + 8 * ws, X0 * L, Y0, zs + q - 2 * R, 0);
                         }
                     }
                 }
             }
         }
-        if (lane0) bulk_wait_read<0>();  // the staging rows must outlive the stores that read them
+#undef FD6_STEP
     }
 };
 
 template <class T, bool PATH55, int TX, int TY>
 __global__ void __launch_bounds__(TX* TY, 1)
-    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, int zc) {
-    Tiled<T, PATH55, TX, TY>::run(m, g, c, zc);
+    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, int zc, T* __restrict__ Fout,
+                 T* __restrict__ W, T* __restrict__ Div) {
+    Tiled<T, PATH55, TX, TY>::run(m, g, c, zc, Fout, W, Div);
 }
 
 // Tile shape per value type (registers per thread bound the CTA size).
@@ -422,7 +396,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 
 struct TiledState {
     bool ready = false;
-    Maps maps[2];      // maps[cur]: read copy F[cur], write copy F[1-cur]
+    Maps maps[2];      // maps[cur]: read copy F[cur]
     int zc = 0;        // planes per z chunk
     int sm_count = 0;
     char err[256] = "";
@@ -470,9 +444,9 @@ static int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, long long
     return 0;
 }
 
-// F[0], F[1]: the two padded copies; W: the dense w arrays; Div: the padded div array or NULL (55-point path only).
+// F[0], F[1]: the two padded copies; W: the dense w arrays.
 template <class T>
-static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W, void* Div) {
+static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
     ts.ready = false;
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
     void* F[2] = {F0, F1};
@@ -480,16 +454,7 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
     for (int cur = 0; cur < 2 && rc == 0; ++cur) {
         Maps& m = ts.maps[cur];
         rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TY + 2 * R, 4);
-        // stores clip at the end of the interior in x, so that a ragged tile leaves the pad columns alone
-        if (rc == 0) rc = tiled_make_map<T>(ts, &m.f_out, F[1 - cur], g.gx + g.nx, g.py, g.pz, 4, g.px, g.py, g.fs, 32, 1, 4);
         if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY, 4);
-        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_st, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, 32, 1, 4);
-        if (rc == 0) {
-            if (Div)
-                rc = tiled_make_map<T>(ts, &m.div_st, Div, g.gx + g.nx, g.py, g.pz, 1, g.px, g.py, g.fs, 32, 1, 1);
-            else
-                m.div_st = m.f_out;  // never used on the 55-point path
-        }
     }
     if (rc) return rc;
     cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -568,13 +533,14 @@ static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
 // Launch of the main kernel of one substep (fused 55-point kernel, or pass 1 of the 19-point path, which
 // leaves dt * div u in Div): reads copy `cur`, writes copy 1 - cur and w.
 template <class T>
-static int tiled_launch_main(TiledState& ts, int path55, int cur, const Geom& g, const KC<T>& c, cudaStream_t stream) {
+static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
+                             cudaStream_t stream) {
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
     dim3 block(TX, TY, 1), grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + ts.zc - 1) / ts.zc);
     if (path55)
-        k_tiled_main<T, true, TX, TY><<<grid, block, Tiled<T, true, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc);
+        k_tiled_main<T, true, TX, TY><<<grid, block, Tiled<T, true, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
     else
-        k_tiled_main<T, false, TX, TY><<<grid, block, Tiled<T, false, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc);
+        k_tiled_main<T, false, TX, TY><<<grid, block, Tiled<T, false, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 
