@@ -36,7 +36,10 @@ UNIT = "Mcell-updates/s"
 WORDS_PER_CELL_SUBSTEP = {"55": 16, "19": 30}  # SURVEY.md 8(d), DESIGN.md "Kernels"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at C4, from the committed
 # `ncu --set full` capture (profiles/); None until that capture exists for the kernel bench.py times.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r01_ncu_fused55_paired_v4_C4.md, launch B (the substep that reads and writes w)
+    ("C4", "fused55"): 9.086e9,
+}
 
 
 def _env_int(name, default):
@@ -321,7 +324,7 @@ def main():
             "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {n}^3 periodic {cfg.dtype}, band-limited |k|<={cfg.kmax} rms Mach {cfg.amp}, "
                                    f"nu={cfg.nu}, dt=0.1 dx/cs", "path": f"{args.path}-point",
-                       "variant": {1: "direct", 2: "tiled"}.get(info.variant, str(info.variant)),
+                       "variant": {1: "direct", 2: "tiled", 3: "paired"}.get(info.variant, str(info.variant)),
                        "l2": "inputs larger than L2 (2.1 GB state, 8.6 GB streamed per substep); no flush needed",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
