@@ -11,14 +11,17 @@
 //   out  F_out, w (and div u) go straight from registers to global memory: a warp writes one 256-byte row
 //        segment per array.  (Staging them in shared memory for TMA box stores was measured 5-11 % slower: the
 //        kernel is bound by shared-memory bandwidth.)
-// Each thread owns one column and keeps everything that couples planes in registers:
+// Each thread owns one column and keeps everything that couples planes thread-private:
 //   win[f][8]   sliding window of its own column along z                     -> D1z, D2z          (Eq. 6, 7)
+//               (8-byte value types: in TENSOR MEMORY, one tcgen05.st of the new plane and one 16-column
+//               tcgen05.ld per field and plane; plain fp32: in registers)
 //   lin[i][8]   accumulator ring of everything of dt*rhs_i that is known when a plane is staged: the in-plane
 //               second derivatives (D2x, D2y, Dxy), the in-plane part of the nonlinear terms, and the mixed
 //               derivatives that involve z (Eq. 8), which are formed from the in-plane differences
 //               f(x+m) - f(x-m) that D1x / D1y need anyway:  Dxz f(z) = sum_m c_m [dx_m f(z+m) - dx_m f(z-m)],
 //               so plane t scatters +-c_m dx_m into the ring slots of outputs t-m and t+m (no extra loads)
-//   dl[6][4]    the six in-plane quantities that multiply z derivatives, delayed until their plane is the centre.
+//   and parks in TENSOR MEMORY (tcgen05.st / tcgen05.ld; idle otherwise, there is no tensor-core work here) the
+//   six in-plane quantities that multiply z derivatives, until their plane is the centre three planes later.
 // Output plane z = t-3 is finished (Eq. 1-3) and updated (Eq. 10) when plane t = z+3 has been consumed.
 // dt is folded into the velocity-derivative coefficients, so the kernel forms dt*rhs directly.
 // The accumulation order of every output depends only on relative plane index, never on the position in a
@@ -84,36 +87,139 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tm,
         "l"(tm), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
         : "memory");
 }
-template <class T, bool PATH55, int TX, int TY>
+
+// ---- tensor memory as a per-thread delay line (tcgen05.st / tcgen05.ld, shape 32x32b: lane = thread of the
+// warp's quadrant, consecutive 32-bit columns).  TMEM is otherwise idle in this kernel (no tensor-core work);
+// parking the six delayed in-plane values of the last three planes there frees 36 registers per thread.
+template <int N>
+__device__ __forceinline__ void tmem_st(uint32_t taddr, const uint32_t* r) {
+    static_assert(N == 2 || N == 4 || N == 8, "chunk size");
+    if constexpr (N == 8)
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]),
+                     "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+                     : "memory");
+    else if constexpr (N == 4)
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3])
+                     : "memory");
+    else
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void tmem_ld(uint32_t taddr, uint32_t* r) {
+    static_assert(N == 2 || N == 4 || N == 8, "chunk size");
+    if constexpr (N == 8)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                     : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                     : "r"(taddr)
+                     : "memory");
+    else if constexpr (N == 4)
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr) : "memory");
+    else
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* r) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// six values of T <-> 6 * sizeof(T) / 4 registers
+template <class T>
+struct Regs6 {
+    static constexpr int N = 6 * (int)sizeof(T) / 4;
+    static __device__ __forceinline__ void pack(const T v[6], uint32_t* r) {
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            if constexpr (sizeof(T) == 4) {
+                r[i] = __float_as_uint(*reinterpret_cast<const float*>(&v[i]));
+            } else {
+                const uint2 u = *reinterpret_cast<const uint2*>(&v[i]);
+                r[2 * i] = u.x;
+                r[2 * i + 1] = u.y;
+            }
+        }
+    }
+    static __device__ __forceinline__ void unpack(const uint32_t* r, T v[6]) {
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+            if constexpr (sizeof(T) == 4) {
+                const float f = __uint_as_float(r[i]);
+                v[i] = *reinterpret_cast<const T*>(&f);
+            } else {
+                const uint2 u = make_uint2(r[2 * i], r[2 * i + 1]);
+                v[i] = *reinterpret_cast<const T*>(&u);
+            }
+        }
+    }
+    static __device__ __forceinline__ void store(uint32_t taddr, const T v[6]) {
+        uint32_t r[N];
+        pack(v, r);
+        if constexpr (N == 12) {
+            tmem_st<8>(taddr, r);
+            tmem_st<4>(taddr + 8, r + 8);
+        } else {
+            tmem_st<4>(taddr, r);
+            tmem_st<2>(taddr + 4, r + 4);
+        }
+    }
+    static __device__ __forceinline__ void load(uint32_t taddr, T v[6]) {
+        uint32_t r[N];
+        if constexpr (N == 12) {
+            tmem_ld<8>(taddr, r);
+            tmem_ld<4>(taddr + 8, r + 8);
+        } else {
+            tmem_ld<4>(taddr, r);
+            tmem_ld<2>(taddr + 4, r + 4);
+        }
+        tmem_wait_ld();
+        unpack(r, v);
+    }
+};
+
+template <class T, bool PATH55, int TX, int TY, int NS_>
 struct Tiled {
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
     static constexpr int PYS = TY + 2 * R;
     static constexpr int FIELD = PXS * PYS;
     static constexpr int STAGE = 4 * FIELD;  // values per stage: four fields of one plane
-    static constexpr int NS = 8;             // stages = unroll factor of the plane loop: stage offsets are immediates
+    static constexpr int NS = NS_;           // stages (4 or 8); the plane loop is unrolled 8x, so stage offsets are immediates
+    static_assert(NS == 4 || NS == 8, "ring depth");
+    static constexpr int LNS = NS == 8 ? 3 : 2;
     static constexpr int NW = 4;             // w stages
     static constexpr int WFIELD = TX * TY;
     static constexpr int WSTAGE = 4 * WFIELD;
     static constexpr int THREADS = TX * TY;
     static constexpr int WARPS = THREADS / 32;
-    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW) * sizeof(uint64_t);
+    // Tensor memory as per-thread storage (8-byte value types): a warp owns the 32 lanes of its quadrant (warp % 4);
+    // the warps of a quadrant use different column blocks.  Block = 4 delay-line slots of 16 columns (6 values) +
+    // 4 fields x 8 window slots of 2 columns = 128 columns.  TMEM is otherwise idle here: no tensor-core work.
+    static constexpr bool TM = sizeof(T) == 8;
+    static constexpr int DLCOLS = 16, TWIN = 4 * DLCOLS, TBLOCK = TWIN + 4 * 16;
+    static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * TBLOCK;
+    static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
+    static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 1) * sizeof(uint64_t);
     static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
     struct State {
         T win[4][8];
         T lin[3][8];
-        T dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 — of the last planes
+        T dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of the last planes (registers: !TM only)
     };
 
     // One plane.  sp0: this thread's centre in stage 0 of the F ring; wsp0: its element in stage 0 of the w ring;
     // gF, gW, gD: its cell of output plane z = t - 3 in F_out, w and div (field strides fs, n); `out`: that plane
     // is produced; store_ok: the thread's column lies inside the grid.
     template <int PH>
-    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const T* __restrict__ wsp0, const KC<T>& c,
-                                                bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
+    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
+                                                const KC<T>& c, bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
                                                 long long n, bool store_ok) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
-        const T* sp = sp0 + n8 * STAGE;
+        const T* sp = sp0 + (PH & (NS - 1)) * STAGE;
         // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8)
         T ctr[4], d1x[4], d1y[4], inpl[3];
         T ex[3], ey[3], ez[3];  // the differences that feed Dxz u_z, Dyz u_z, Dzx u_x + Dzy u_y
@@ -121,7 +227,13 @@ struct Tiled {
         for (int f = 0; f < 4; ++f) {
             const T* q = sp + f * FIELD;
             ctr[f] = q[0];
-            st.win[f][n8] = ctr[f];
+            if constexpr (TM) {
+                const uint2 u = *reinterpret_cast<const uint2*>(&ctr[f]);
+                const uint32_t r2[2] = {u.x, u.y};
+                tmem_st<2>(tdl + TWIN + f * 16 + n8 * 2, r2);
+            } else {
+                st.win[f][n8] = ctr[f];
+            }
             const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
             const T yp1 = q[PXS], ym1 = q[-PXS], yp2 = q[2 * PXS], ym2 = q[-2 * PXS], yp3 = q[3 * PXS], ym3 = q[-3 * PXS];
             const T dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
@@ -195,17 +307,46 @@ struct Tiled {
 #pragma unroll
                 for (int i = 0; i < 3; ++i) st.lin[i][n8] = pl[i];
             }
-            st.dl[0][n4] = gx;
-            st.dl[1][n4] = gy;
-            st.dl[2][n4] = Gzx;
-            st.dl[3][n4] = Gzy;
-            st.dl[4][n4] = Dh;
-            st.dl[5][n4] = P0;
+            // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of plane t -> delay-line slot t & 3
+            if constexpr (TM) {
+                const T park[6] = {gx, gy, Gzx, Gzy, Dh, P0};
+                Regs6<T>::store(tdl + n4 * DLCOLS, park);
+            } else {
+                st.dl[0][n4] = gx;
+                st.dl[1][n4] = gy;
+                st.dl[2][n4] = Gzx;
+                st.dl[3][n4] = Gzy;
+                st.dl[4][n4] = Dh;
+                st.dl[5][n4] = P0;
+            }
         }
         if (!out) return;
         // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
         constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
-        T d1z[4], fc[4];
+        T d1z[4], fc[4], del[6];
+        if constexpr (TM) {
+            // the whole window ring of a field is 16 consecutive columns: one load each; slot t of this plane may
+            // still be in flight, so it is taken from the register that holds it
+            uint32_t wr[4][16], dr[12];
+#pragma unroll
+            for (int f = 0; f < 4; ++f) tmem_ld16(tdl + TWIN + f * 16, wr[f]);
+            tmem_ld<8>(tdl + r4 * DLCOLS, dr);
+            tmem_ld<4>(tdl + r4 * DLCOLS + 8, dr + 8);
+            tmem_wait_ld();
+#pragma unroll
+            for (int f = 0; f < 4; ++f) {
+#pragma unroll
+                for (int a8 = 0; a8 < 8; ++a8) {
+                    const uint2 u = make_uint2(wr[f][2 * a8], wr[f][2 * a8 + 1]);
+                    st.win[f][a8] = *reinterpret_cast<const T*>(&u);
+                }
+                st.win[f][n8] = ctr[f];
+            }
+            Regs6<T>::unpack(dr, del);
+        } else {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) del[q] = st.dl[q][r4];
+        }
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
             const T* a = f == 0 ? c.ar : c.au;
@@ -224,7 +365,7 @@ struct Tiled {
             v = fma_(bz[3], st.win[f][(cz + 3) & 7] + st.win[f][(cz + 5) & 7], v);
             lz[i] = v;
         }
-        const T gxd = st.dl[0][r4], gyd = st.dl[1][r4], Gzxd = st.dl[2][r4], Gzyd = st.dl[3][r4], Dhd = st.dl[4][r4], P0d = st.dl[5][r4];
+        const T gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
         const T gz = d1z[0], Gxz = d1z[1], Gyz = d1z[2], Gzz = d1z[3], uz = fc[3];
         const T divp = Dhd + Gzz;  // dt * div u
         T Rv[4];
@@ -286,7 +427,22 @@ struct Tiled {
             for (int i = 0; i < NW; ++i) mbar_init(a_wfull + 8 * i, 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
-        __syncthreads();
+        const uint32_t a_tmem = a_wfull + 8 * NW;  // shared word that receives the TMEM base address
+        uint32_t tmem_base = 0;
+        if constexpr (TM) {
+            if (tid < 32) {  // warp 0 allocates (and frees) the tensor-memory columns
+                asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(a_tmem), "n"(TMEM_COLS) : "memory");
+                asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+            }
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(a_tmem) : "memory");
+        } else {
+            __syncthreads();
+        }
+        // a warp reaches the 32 lanes of its quadrant (warp % 4); warps that share a quadrant use different columns
+        const uint32_t tdl = tmem_base + ((uint32_t)(((tid >> 5) & 3) * 32) << 16) + (uint32_t)((tid >> 7) * TBLOCK);
         if (producer) {
             for (int i = 0; i < NS && i < np; ++i) {
                 mbar_expect_tx(a_full + 8 * i, kStageBytes);
@@ -321,9 +477,10 @@ struct Tiled {
                 const int p = pb + ph;
                 if (p < np) {
                     const bool out = p >= 2 * R;  // planes 0..5 of a chunk only warm the window and the rings up
-                    mbar_wait(a_full + 8 * ph, (uint32_t)((p >> 3) & 1));
+                    if constexpr (TM) tmem_wait_st();  // what the previous planes parked in tensor memory is in place
+                    mbar_wait(a_full + 8 * (ph & (NS - 1)), (uint32_t)((p >> LNS) & 1));
                     if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
-#define FD6_STEP(K) step<K>(st, sp0, wsp0, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, store_ok)
+#define FD6_STEP(K) step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, store_ok)
                     switch (ph) {  // ph is a compile-time constant after unrolling
                         case 0: FD6_STEP(0); break;
                         case 1: FD6_STEP(1); break;
@@ -340,15 +497,15 @@ struct Tiled {
                     }
                     // this warp is done reading stage ph (F) and its w slot: hand them back
                     __syncwarp();
-                    if (lane0) mbar_arrive(a_empty + 8 * ph);
+                    if (lane0) mbar_arrive(a_empty + 8 * (ph & (NS - 1)));
                     // thread 0 refills the stage every warp has released one plane earlier, so it never waits for a
                     // warp that is less than a plane behind; the w values of step q = p + 3 go into the slot step p - 1 used
                     if (producer && p >= 1) {
-                        const int sprev = (ph + 7) & 7;
+                        const int sprev = (ph + 7) & (NS - 1);
                         const bool more_f = p - 1 + NS < np;
                         const int q = p + 3;
                         const bool more_w = c.read_w && q >= 2 * R && q < np;
-                        if (more_f || more_w) mbar_wait(a_empty + 8 * sprev, (uint32_t)(((p - 1) >> 3) & 1));
+                        if (more_f || more_w) mbar_wait(a_empty + 8 * sprev, (uint32_t)(((p - 1) >> LNS) & 1));
                         if (more_f) {
                             mbar_expect_tx(a_full + 8 * sprev, kStageBytes);
                             tma_load_4d(a_sm + sprev * kStageBytes, &m.f_in, a_full + 8 * sprev, bx, by, bz + p - 1 + NS, 0);
@@ -363,14 +520,19 @@ struct Tiled {
             }
         }
 #undef FD6_STEP
+        if constexpr (TM) {
+            asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+            __syncthreads();
+            if (tid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TMEM_COLS) : "memory");
+        }
     }
 };
 
-template <class T, bool PATH55, int TX, int TY>
+template <class T, bool PATH55, int TX, int TY, int NS>
 __global__ void __launch_bounds__(TX* TY, 1)
     k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, int zc, T* __restrict__ Fout,
                  T* __restrict__ W, T* __restrict__ Div) {
-    Tiled<T, PATH55, TX, TY>::run(m, g, c, zc, Fout, W, Div);
+    Tiled<T, PATH55, TX, TY, NS>::run(m, g, c, zc, Fout, W, Div);
 }
 
 // Tile shape per value type (registers per thread bound the CTA size).
@@ -378,15 +540,15 @@ template <class T>
 struct TileShape;
 template <>
 struct TileShape<float> {
-    static constexpr int TX = 64, TY = 8;
+    static constexpr int TX = 64, TY = 8, NS = 8;  // 16 warps x 128 registers, state in registers
 };
 template <>
 struct TileShape<double> {
-    static constexpr int TX = 32, TY = 8;
+    static constexpr int TX = 32, TY = 8, NS = 4;  // 8 warps; window and delay line in tensor memory (12 warps measured slower: DFMA-bound)
 };
 template <>
 struct TileShape<V2> {
-    static constexpr int TX = 32, TY = 8;
+    static constexpr int TX = 32, TY = 12, NS = 4;  // 12 warps x <= 168 registers: window and delay line in tensor memory
 };
 
 // ---- host side -------------------------------------------------------------------------------------------
@@ -448,7 +610,7 @@ static int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, long long
 template <class T>
 static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
     ts.ready = false;
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS;
     void* F[2] = {F0, F1};
     int rc = 0;
     for (int cur = 0; cur < 2 && rc == 0; ++cur) {
@@ -457,11 +619,11 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
         if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY, 4);
     }
     if (rc) return rc;
-    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Tiled<T, true, TX, TY>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)Tiled<T, true, TX, TY, NS>::SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Tiled<T, false, TX, TY>::SMEM);
+        e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)Tiled<T, false, TX, TY, NS>::SMEM);
     if (e != cudaSuccess) {
         snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
         cudaGetLastError();
@@ -535,12 +697,12 @@ static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
 template <class T>
 static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
                              cudaStream_t stream) {
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY;
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS;
     dim3 block(TX, TY, 1), grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + ts.zc - 1) / ts.zc);
     if (path55)
-        k_tiled_main<T, true, TX, TY><<<grid, block, Tiled<T, true, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
+        k_tiled_main<T, true, TX, TY, NS><<<grid, block, Tiled<T, true, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
     else
-        k_tiled_main<T, false, TX, TY><<<grid, block, Tiled<T, false, TX, TY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
+        k_tiled_main<T, false, TX, TY, NS><<<grid, block, Tiled<T, false, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 
