@@ -49,6 +49,16 @@ struct KC {
     int read_w, write_f, write_w;
 };
 
+// Work list of one launch (1-D grid, one CTA per item, launched in this order).  The first n_full tiles (a
+// multiple of the SM count) are marched through all of z by one CTA each; the remaining tiles, which would
+// fill only part of a last wave, are cut into k z-chunks of zc planes so that their items fill whole waves
+// again (each chunk re-stages 6 warm-up planes, which is why only the remainder is cut).
+struct Sched {
+    int ntx;     // tiles along x; tile index = bx + ntx * by
+    int n_full;  // tiles with a single item
+    int k, zc;   // chunks per remaining tile, planes per chunk
+};
+
 // The tensor maps of one launch (each 128 bytes, passed by value as a __grid_constant__ parameter).
 struct Maps {
     CUtensorMap f_in;  // padded fields, read copy: box (TX+8, TY+6, 1, 4)
@@ -398,7 +408,7 @@ struct Tiled {
         }
     }
 
-    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, int zc, T* __restrict__ Fout,
+    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, const Sched sc, T* __restrict__ Fout,
                                                T* __restrict__ W, T* __restrict__ Div) {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
@@ -409,8 +419,15 @@ struct Tiled {
         const int tx = threadIdx.x, ty = threadIdx.y;
         const int tid = ty * TX + tx;
         const bool lane0 = (tid & 31) == 0, producer = tid == 0;
-        const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
-        const int zs = blockIdx.z * zc, ze = min(zs + zc, g.nz);
+        int tile = blockIdx.x, zs = 0, ze = g.nz;
+        if (tile >= sc.n_full) {
+            const int j = tile - sc.n_full;
+            tile = sc.n_full + j / sc.k;
+            zs = (j % sc.k) * sc.zc;
+            ze = min(zs + sc.zc, g.nz);
+        }
+        if (zs >= ze) return;  // empty chunk (rounding); the whole CTA leaves before any barrier
+        const int X0 = (tile % sc.ntx) * TX, Y0 = (tile / sc.ntx) * TY;
         const int np = ze - zs + 2 * R;  // staged planes t = zs-3 .. ze+2
         constexpr int L = Scalar<T>::lanes;
         // TMA box origin; the tensor maps count scalars along x, a value is L of them
@@ -530,9 +547,9 @@ struct Tiled {
 
 template <class T, bool PATH55, int TX, int TY, int NS>
 __global__ void __launch_bounds__(TX* TY, 1)
-    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, int zc, T* __restrict__ Fout,
+    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, const Sched sc, T* __restrict__ Fout,
                  T* __restrict__ W, T* __restrict__ Div) {
-    Tiled<T, PATH55, TX, TY, NS>::run(m, g, c, zc, Fout, W, Div);
+    Tiled<T, PATH55, TX, TY, NS>::run(m, g, c, sc, Fout, W, Div);
 }
 
 // Tile shape per value type (registers per thread bound the CTA size).
@@ -559,7 +576,8 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 struct TiledState {
     bool ready = false;
     Maps maps[2];      // maps[cur]: read copy F[cur]
-    int zc = 0;        // planes per z chunk
+    Sched sched{};     // work list
+    int items = 0;     // grid size
     int sm_count = 0;
     char err[256] = "";
 };
@@ -633,23 +651,28 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
-    // z chunking: one CTA per SM is resident; pick the number of chunks that fills whole waves of SMs best while
-    // keeping the 6-plane warm-up of every chunk small.
-    const long long tiles = (long long)((g.nx + TX - 1) / TX) * ((g.ny + TY - 1) / TY);
-    int best_c = 1;
+    // Work list (see Sched): one CTA per SM is resident, so whole waves of sm_count tiles run as full columns and
+    // the remainder is cut into the number of z-chunks that minimises (waves x planes staged per item).
+    const int ntx = (g.nx + TX - 1) / TX, nty = (g.ny + TY - 1) / TY;
+    const int tiles = ntx * nty, S = ts.sm_count;
+    const int n_full = (tiles / S) * S, rem = tiles - n_full;
+    int best_k = 1;
     double best_cost = 1e300;
-    for (int cks = 1; cks <= (g.nz + 7) / 8 && cks <= 64; ++cks) {
-        const int zc = (g.nz + cks - 1) / cks;
+    for (int k = 1; rem > 0 && k <= (g.nz + 7) / 8 && k <= 64; ++k) {
+        const int zc = (g.nz + k - 1) / k;
         const int real = (g.nz + zc - 1) / zc;
-        const long long ctas = tiles * real;
-        const long long waves = (ctas + ts.sm_count - 1) / ts.sm_count;
-        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per CTA (+ fill latency)
+        const long long waves = ((long long)rem * real + S - 1) / S;
+        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per item (+ fill latency)
         if (cost < best_cost) {
             best_cost = cost;
-            best_c = cks;
+            best_k = k;
         }
     }
-    ts.zc = (g.nz + best_c - 1) / best_c;
+    ts.sched.ntx = ntx;
+    ts.sched.n_full = n_full;
+    ts.sched.zc = (g.nz + best_k - 1) / best_k;
+    ts.sched.k = (g.nz + ts.sched.zc - 1) / ts.sched.zc;
+    ts.items = n_full + rem * ts.sched.k;
     ts.ready = true;
     return 0;
 }
@@ -698,11 +721,11 @@ template <class T>
 static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
                              cudaStream_t stream) {
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS;
-    dim3 block(TX, TY, 1), grid((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, (g.nz + ts.zc - 1) / ts.zc);
+    dim3 block(TX, TY, 1), grid(ts.items, 1, 1);
     if (path55)
-        k_tiled_main<T, true, TX, TY, NS><<<grid, block, Tiled<T, true, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
+        k_tiled_main<T, true, TX, TY, NS><<<grid, block, Tiled<T, true, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
     else
-        k_tiled_main<T, false, TX, TY, NS><<<grid, block, Tiled<T, false, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.zc, Fout, W, Div);
+        k_tiled_main<T, false, TX, TY, NS><<<grid, block, Tiled<T, false, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 
