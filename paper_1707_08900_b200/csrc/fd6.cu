@@ -247,7 +247,7 @@ static int launch_halo(fd_ctx* c, T* F, int nfields) {
     const Geom& g = c->g;
     {
         LaunchScope ls(c, FD_K_HALO_X);
-        long long threads = (long long)g.ny * g.nz * nfields;
+        long long threads = 2LL * g.ny * g.nz * nfields;
         k_halo_x<T><<<(unsigned)((threads + 127) / 128), 128, 0, c->stream>>>(F, g, nfields);
     }
     {

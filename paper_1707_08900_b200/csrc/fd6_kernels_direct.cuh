@@ -54,25 +54,30 @@ __global__ void __launch_bounds__(128)
 // ------------------------------------------------------------------------------------------------
 // a1 / a7  periodic halo fill, radius 3 (Alg. 2/3 "Compute boundary conditions").
 //   (T = V2: the stored grid has nz/2 planes and z-periodicity swaps the halves of a pair, see zwrap.)
-//   k_halo_x : every interior row (j,k) copies 3 cells to each x ghost.          thread per (row, field)
+//   k_halo_x : every interior row (j,k) copies one 32-byte sector to each x ghost pad.   thread per (row, side, field)
 //   k_halo_yz: every ghost ROW (j or k outside the domain) is the x-extended copy of the interior row it
 //              wraps to; run after k_halo_x so edge ghosts (two coordinates outside, needed by the Eq. 8
 //              diagonals) come along.  Corner ghosts are filled too (never read).
 // ------------------------------------------------------------------------------------------------
 template <class T>
 __global__ void __launch_bounds__(128) k_halo_x(T* __restrict__ F, Geom g, int nfields) {
+    // One thread per (row, side).  The x ghost pad is exactly one 32-byte sector (gx values) and rows are 32-byte
+    // aligned, so a side is one aligned sector copy: the low pad [0, gx) takes the last gx interior values, the high
+    // pad [gx+nx, 2gx+nx) the first gx (only the R values next to the interior are ever read).
     long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+    const int side = (int)(t & 1);
+    t >>= 1;
     long long rows = (long long)g.ny * g.nz;
     if (t >= rows * nfields) return;
     int q = (int)(t / rows);
     long long r = t - q * rows;
     int j = (int)(r % g.ny), k = (int)(r / g.ny);
-    T* row = F + q * g.fs + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz)) + g.gx;
-#pragma unroll
-    for (int m = 0; m < R; ++m) {
-        row[-1 - m] = row[g.nx - 1 - m];
-        row[g.nx + m] = row[m];
-    }
+    T* row = F + q * g.fs + (long long)g.px * ((j + g.gy) + (long long)g.py * (k + g.gz));
+    const uint4* src = reinterpret_cast<const uint4*>(side ? row + g.gx : row + g.nx);
+    uint4* dst = reinterpret_cast<uint4*>(side ? row + g.gx + g.nx : row);
+    const uint4 a = src[0], b = src[1];
+    dst[0] = a;
+    dst[1] = b;
 }
 
 template <class T>
