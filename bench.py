@@ -211,6 +211,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_1707_08900_b200 import fd6  # raises if libfd6.so is missing: no CPU fallback
+    from paper_1707_08900_b200 import replicas
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (the product path has no CPU fallback)"
     rank, world, local = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
@@ -222,9 +223,10 @@ def main():
     esize = 4 if cfg.dtype == "f32" else 8
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        replicas.barrier("cuda")
+
+    def max_ms(ms_):
+        return replicas.max_over_ranks(ms_, "cuda")
 
     # seeded synthetic state, generated on the device (harness only) then handed to fd_load
     F0 = inputs.make_state(cfg, device="cuda")
@@ -258,11 +260,8 @@ def main():
     ctx.fd_sync()
     finite = bool(torch.isfinite(chk).all().item())
     del chk
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * N * K / (ms_max * 1e-3) / 1e6
+    ms_max = max_ms(ms)
+    value = replicas.whole_job_value(N, K, ms_max, world)
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region
     host_in = torch.empty(F0.shape, dtype=F0.dtype, pin_memory=True)
@@ -281,11 +280,8 @@ def main():
     e2e_job(K)
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item())
-    e2e_value = world * N * K / (e2e_ms * 1e-3) / 1e6
+    e2e_ms = max_ms(e0.elapsed_time(e1))
+    e2e_value = replicas.whole_job_value(N, K, e2e_ms, world)
     reps = 3
     barrier()
     e0.record(stream)
@@ -293,10 +289,7 @@ def main():
         e2e_job(1)
     e1.record(stream)
     barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_each = world * N * reps / (float(t.item()) * 1e-3) / 1e6
+    e2e_each = replicas.whole_job_value(N, reps, max_ms(e0.elapsed_time(e1)), world)
     finite = finite and bool(torch.isfinite(host_out).all().item())
 
     # ---- roofline of the dominant kernel

@@ -6,5 +6,6 @@ compressible hydrodynamics, 2N-storage RK3).
                                 CPU fallback anywhere in this package.
   paper_1707_08900_b200.inputs  seeded synthetic inputs (no method arithmetic).
   paper_1707_08900_b200.build   nvcc build of libfd6.so for sm_100a.
+  paper_1707_08900_b200.replicas  barrier / max-over-ranks bookkeeping of the "replicas only" multi-GPU mode.
 """
-__all__ = ["inputs", "build", "fd6"]
+__all__ = ["inputs", "build", "fd6", "replicas"]
