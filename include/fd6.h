@@ -117,6 +117,18 @@ typedef struct fd_info {
 } fd_info;
 int fd_get_info(const fd_ctx* ctx, fd_info* out);
 
+/* Work list of the tiled kernels (host arithmetic only, needs no CUDA device): the grid is cut
+ * into tiles_x * tiles_y columns of tile_x * tile_y values and `planes` stored planes (nz, or nz/2 in the paired
+ * fp32 layout that FD_VARIANT_AUTO picks for even nz).  Item b of the 1-D launch grid is, for b < full_tiles, tile b
+ * over all planes; otherwise, with j = b - full_tiles, tile full_tiles + j / chunks over planes
+ * [(j % chunks) * chunk_planes, min(that + chunk_planes, planes)).  Every (tile, plane) is covered exactly once.
+ * FD_EINVAL: out == NULL, n < 8, sm_count < 1, bad dtype. */
+typedef struct fd_work_list {
+    int tile_x, tile_y, tiles_x, tiles_y, planes;
+    int full_tiles, chunks, chunk_planes, items;
+} fd_work_list;
+int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count, fd_work_list* out);
+
 /* Number of kernels this context has launched since creation (every kernel of the library counts). */
 unsigned long long fd_kernel_launches(const fd_ctx* ctx);
 

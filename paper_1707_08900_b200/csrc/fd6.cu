@@ -695,6 +695,38 @@ extern "C" int fd_reset_profile(fd_ctx* c) {
     return FD_OK;
 }
 
+// Host-only: the work list the tiled kernels would run for a grid (no CUDA call, usable without a device).
+extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count, fd_work_list* o) {
+    if (!o) return fail(FD_EINVAL, "fd_plan_work_list: out is NULL");
+    if (nx < 8 || ny < 8 || nz < 8 || sm_count < 1) return fail(FD_EINVAL, "fd_plan_work_list: bad grid or SM count");
+    if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_plan_work_list: bad dtype %d", dtype);
+    const bool paired = dtype == FD_F32 && nz % 2 == 0 && nz / 2 >= 4;  // what FD_VARIANT_AUTO resolves to
+    int tx, ty;
+    if (dtype == FD_F64) {
+        tx = TileShape<double>::TX;
+        ty = TileShape<double>::TY;
+    } else if (paired) {
+        tx = TileShape<V2>::TX;
+        ty = TileShape<V2>::TY;
+    } else {
+        tx = TileShape<float>::TX;
+        ty = TileShape<float>::TY;
+    }
+    const int planes = paired ? nz / 2 : nz;
+    int items = 0;
+    const Sched sc = plan_work_list((nx + tx - 1) / tx, (ny + ty - 1) / ty, planes, sm_count, &items);
+    o->tile_x = tx;
+    o->tile_y = ty;
+    o->tiles_x = sc.ntx;
+    o->tiles_y = (ny + ty - 1) / ty;
+    o->planes = planes;
+    o->full_tiles = sc.n_full;
+    o->chunks = sc.k;
+    o->chunk_planes = sc.zc;
+    o->items = items;
+    return FD_OK;
+}
+
 template <class T>
 static int do_poison(fd_ctx* c, bool ghosts) {
     const T nan = T(typename Scalar<T>::type(NAN));

@@ -624,6 +624,33 @@ static int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, long long
     return 0;
 }
 
+// Work list (see Sched; pure host arithmetic, also reachable through fd_plan_work_list for the CPU tests): one CTA
+// per SM is resident, so whole waves of S tiles run as full columns and the remaining tiles are cut into the
+// number of z-chunks that minimises (waves x planes staged per item).
+inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
+    const int tiles = ntx * nty;
+    const int n_full = (tiles / S) * S, rem = tiles - n_full;
+    int best_k = 1;
+    double best_cost = 1e300;
+    for (int k = 1; rem > 0 && k <= (nz + 7) / 8 && k <= 64; ++k) {
+        const int zc = (nz + k - 1) / k;
+        const int real = (nz + zc - 1) / zc;
+        const long long waves = ((long long)rem * real + S - 1) / S;
+        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per item (+ fill latency)
+        if (cost < best_cost) {
+            best_cost = cost;
+            best_k = k;
+        }
+    }
+    Sched sc;
+    sc.ntx = ntx;
+    sc.n_full = n_full;
+    sc.zc = (nz + best_k - 1) / best_k;
+    sc.k = (nz + sc.zc - 1) / sc.zc;
+    *items = n_full + rem * sc.k;
+    return sc;
+}
+
 // F[0], F[1]: the two padded copies; W: the dense w arrays.
 template <class T>
 static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
@@ -651,28 +678,7 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
-    // Work list (see Sched): one CTA per SM is resident, so whole waves of sm_count tiles run as full columns and
-    // the remainder is cut into the number of z-chunks that minimises (waves x planes staged per item).
-    const int ntx = (g.nx + TX - 1) / TX, nty = (g.ny + TY - 1) / TY;
-    const int tiles = ntx * nty, S = ts.sm_count;
-    const int n_full = (tiles / S) * S, rem = tiles - n_full;
-    int best_k = 1;
-    double best_cost = 1e300;
-    for (int k = 1; rem > 0 && k <= (g.nz + 7) / 8 && k <= 64; ++k) {
-        const int zc = (g.nz + k - 1) / k;
-        const int real = (g.nz + zc - 1) / zc;
-        const long long waves = ((long long)rem * real + S - 1) / S;
-        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per item (+ fill latency)
-        if (cost < best_cost) {
-            best_cost = cost;
-            best_k = k;
-        }
-    }
-    ts.sched.ntx = ntx;
-    ts.sched.n_full = n_full;
-    ts.sched.zc = (g.nz + best_k - 1) / best_k;
-    ts.sched.k = (g.nz + ts.sched.zc - 1) / ts.sched.zc;
-    ts.items = n_full + rem * ts.sched.k;
+    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, g.nz, ts.sm_count, &ts.items);
     ts.ready = true;
     return 0;
 }

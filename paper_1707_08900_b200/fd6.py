@@ -25,6 +25,7 @@ EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
     "fd_rhs", "fd_rk3_step", "fd_sync", "fd_destroy", "fd_last_error", "fd_get_info", "fd_kernel_launches",
     "fd_set_profiling", "fd_get_profile", "fd_reset_profile", "fd_debug_poison_w", "fd_debug_poison_ghosts",
+    "fd_plan_work_list",
 ]
 
 if not os.path.exists(_LIB_PATH):
@@ -40,6 +41,11 @@ class FdInfo(C.Structure):
                 ("variant", C.c_int), ("pitch_x", C.c_int), ("pitch_y", C.c_int), ("pitch_z", C.c_int),
                 ("ghost_x", C.c_int), ("ghost_y", C.c_int), ("ghost_z", C.c_int),
                 ("field_stride", C.c_size_t), ("device_bytes", C.c_size_t)]
+
+
+class FdWorkList(C.Structure):
+    _fields_ = [(n, C.c_int) for n in ("tile_x", "tile_y", "tiles_x", "tiles_y", "planes", "full_tiles", "chunks",
+                                       "chunk_planes", "items")]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)
@@ -66,6 +72,16 @@ lib.fd_get_profile.argtypes = [_vp, _i, C.POINTER(_d), C.POINTER(C.c_ulonglong)]
 lib.fd_reset_profile.argtypes = [_vp]
 lib.fd_debug_poison_w.argtypes = [_vp]
 lib.fd_debug_poison_ghosts.argtypes = [_vp]
+lib.fd_plan_work_list.argtypes = [_i, _i, _i, _i, _i, C.POINTER(FdWorkList)]
+
+
+def fd_plan_work_list(nx, ny, nz, dtype, sm_count):
+    """Work list of the tiled kernels for a grid (host arithmetic only; needs no CUDA device)."""
+    wl = FdWorkList()
+    code = lib.fd_plan_work_list(nx, ny, nz, dtype, sm_count, C.byref(wl))
+    if code != FD_OK:
+        raise FdError(code, lib.fd_last_error().decode())
+    return wl
 
 
 class FdError(RuntimeError):

@@ -81,3 +81,51 @@ def test_no_cpu_fallback_without_a_device(fd6):
     assert b"no CPU fallback" in fd6.lib.fd_last_error()
     with pytest.raises(fd6.FdError):
         fd6.Fd(32, 32, 32, 0.1, 0.0, 1.0)
+
+
+def _items(wl):
+    """Enumerate (tile, plane range) of every launch-grid item exactly as fd6.h documents it."""
+    for b in range(wl.items):
+        if b < wl.full_tiles:
+            yield b, 0, wl.planes
+        else:
+            j = b - wl.full_tiles
+            zs = (j % wl.chunks) * wl.chunk_planes
+            yield wl.full_tiles + j // wl.chunks, zs, min(zs + wl.chunk_planes, wl.planes)
+
+
+@pytest.mark.parametrize("shape", [(512, 512, 512), (256, 256, 256), (128, 128, 128), (32, 32, 32), (1024, 1024, 1024),
+                                   (40, 13, 9), (8, 8, 8), (132, 70, 20), (72, 33, 41), (512, 96, 30), (2048, 8, 8)])
+@pytest.mark.parametrize("dtype", [0, 1])
+@pytest.mark.parametrize("sms", [148, 1, 132, 7])
+def test_work_list_covers_every_tile_plane_exactly_once(fd6, shape, dtype, sms):
+    nx, ny, nz = shape
+    wl = fd6.fd_plan_work_list(nx, ny, nz, dtype, sms)
+    tiles = wl.tiles_x * wl.tiles_y
+    assert wl.tiles_x * wl.tile_x >= nx > (wl.tiles_x - 1) * wl.tile_x
+    assert wl.tiles_y * wl.tile_y >= ny > (wl.tiles_y - 1) * wl.tile_y
+    paired = dtype == 0 and nz % 2 == 0
+    assert wl.planes == (nz // 2 if paired else nz)
+    assert wl.full_tiles % sms == 0 and 0 <= tiles - wl.full_tiles < sms
+    assert wl.items == wl.full_tiles + (tiles - wl.full_tiles) * wl.chunks
+    covered = [0] * (tiles * wl.planes)
+    for tile, zs, ze in _items(wl):
+        assert 0 <= tile < tiles
+        for z in range(zs, ze):  # an empty range (zs >= ze) is an item that returns at once
+            covered[tile * wl.planes + z] += 1
+    assert min(covered) == 1 and max(covered) == 1
+
+
+def test_work_list_of_the_headline_config(fd6):
+    wl = fd6.fd_plan_work_list(512, 512, 512, fd6.FD_F32, 148)
+    # 16 x 43 tiles of 32 x 12 pairs: four full waves of columns, the remaining 96 tiles cut in z (DESIGN.md section 7)
+    assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes, wl.full_tiles) == (32, 12, 16, 43, 256, 592)
+    assert wl.chunks >= 2 and wl.items == 592 + 96 * wl.chunks
+
+
+def test_work_list_rejects_bad_arguments(fd6):
+    wl = fd6.FdWorkList()
+    assert fd6.lib.fd_plan_work_list(512, 512, 512, 0, 148, None) == fd6.FD_EINVAL
+    assert fd6.lib.fd_plan_work_list(4, 512, 512, 0, 148, C.byref(wl)) == fd6.FD_EINVAL
+    assert fd6.lib.fd_plan_work_list(512, 512, 512, 0, 0, C.byref(wl)) == fd6.FD_EINVAL
+    assert fd6.lib.fd_plan_work_list(512, 512, 512, 5, 148, C.byref(wl)) == fd6.FD_EINVAL
