@@ -704,13 +704,13 @@ extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count
     int tx, ty;
     if (dtype == FD_F64) {
         tx = TileShape<double>::TX;
-        ty = TileShape<double>::TY;
+        ty = TileShape<double>::TY * TileShape<double>::RY;
     } else if (paired) {
         tx = TileShape<V2>::TX;
-        ty = TileShape<V2>::TY;
+        ty = TileShape<V2>::TY * TileShape<V2>::RY;
     } else {
         tx = TileShape<float>::TX;
-        ty = TileShape<float>::TY;
+        ty = TileShape<float>::TY * TileShape<float>::RY;
     }
     const int planes = paired ? nz / 2 : nz;
     int items = 0;

@@ -190,106 +190,134 @@ struct Regs6 {
     }
 };
 
-template <class T, bool PATH55, int TX, int TY, int NS_>
+// TX x TY threads; a thread owns RY vertically adjacent columns (rows cj .. cj+RY-1), so the tile is TX x (TY*RY).
+template <class T, bool PATH55, int TX, int TY, int NS_, int RY>
 struct Tiled {
+    static constexpr int TH = TY * RY;  // tile height in values
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
-    static constexpr int PYS = TY + 2 * R;
+    static constexpr int PYS = TH + 2 * R;
     static constexpr int FIELD = PXS * PYS;
     static constexpr int STAGE = 4 * FIELD;  // values per stage: four fields of one plane
     static constexpr int NS = NS_;           // stages (4 or 8); the plane loop is unrolled 8x, so stage offsets are immediates
     static_assert(NS == 4 || NS == 8, "ring depth");
     static constexpr int LNS = NS == 8 ? 3 : 2;
     static constexpr int NW = 4;             // w stages
-    static constexpr int WFIELD = TX * TY;
+    static constexpr int WFIELD = TX * TH;
     static constexpr int WSTAGE = 4 * WFIELD;
     static constexpr int THREADS = TX * TY;
     static constexpr int WARPS = THREADS / 32;
     // Tensor memory as per-thread storage (8-byte value types): a warp owns the 32 lanes of its quadrant (warp % 4);
-    // the warps of a quadrant use different column blocks.  Block = 4 delay-line slots of 16 columns (6 values) +
-    // 4 fields x 8 window slots of 2 columns = 128 columns.  TMEM is otherwise idle here: no tensor-core work.
+    // the warps of a quadrant use different column blocks, one per owned column.  Block = 4 delay-line slots of 16
+    // columns (6 values) + 4 fields x 8 window slots of 2 columns = 128 columns.  TMEM is otherwise idle here.
     static constexpr bool TM = sizeof(T) == 8;
     static constexpr int DLCOLS = 16, TWIN = 4 * DLCOLS, TBLOCK = TWIN + 4 * 16;
-    static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * TBLOCK;
+    static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * RY * TBLOCK;
     static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
     static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
     static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 1) * sizeof(uint64_t);
     static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
-    struct State {
+    struct State {   // of one owned column
         T win[4][8];
         T lin[3][8];
         T dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of the last planes (registers: !TM only)
     };
 
-    // One plane.  sp0: this thread's centre in stage 0 of the F ring; wsp0: its element in stage 0 of the w ring;
-    // gF, gW, gD: its cell of output plane z = t - 3 in F_out, w and div (field strides fs, n); `out`: that plane
-    // is produced; store_ok: the thread's column lies inside the grid.
+    // scatter of the in-plane differences e_m of plane t into the accumulator ring of one rhs component (Eq. 8 with z)
+    template <int n8>
+    static __device__ __forceinline__ void scatter(T (&lin)[8], const T (&e)[3], const KC<T>& c) {
+        lin[(n8 + 3) & 7] = -(c.mq[2] * e[2]);  // first contribution to output t+3
+        lin[(n8 + 2) & 7] = fma_(-c.mq[1], e[1], lin[(n8 + 2) & 7]);
+        lin[(n8 + 1) & 7] = fma_(-c.mq[0], e[0], lin[(n8 + 1) & 7]);
+        lin[(n8 + 7) & 7] = fma_(c.mq[0], e[0], lin[(n8 + 7) & 7]);
+        lin[(n8 + 6) & 7] = fma_(c.mq[1], e[1], lin[(n8 + 6) & 7]);
+        lin[(n8 + 5) & 7] = fma_(c.mq[2], e[2], lin[(n8 + 5) & 7]);  // output t-3 is complete
+    }
+
+    // One plane.  sp0: the thread's first centre in stage 0 of the F ring; wsp0: its first element in stage 0 of the
+    // w ring; gF, gW, gD: its first cell of output plane z = t - 3 in F_out, w and div (field strides fs, n; row
+    // pitches pf, pw); `out`: that plane is produced; ok[r]: owned column r lies inside the grid.
     template <int PH>
-    static __device__ __forceinline__ void step(State& st, const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
+    static __device__ __forceinline__ void step(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
                                                 const KC<T>& c, bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
-                                                long long n, bool store_ok) {
+                                                long long n, int pf, int pw, const bool (&ok)[RY]) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
         const T* sp = sp0 + (PH & (NS - 1)) * STAGE;
-        // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8)
-        T ctr[4], d1x[4], d1y[4], inpl[3];
-        T ex[3], ey[3], ez[3];  // the differences that feed Dxz u_z, Dyz u_z, Dzx u_x + Dzy u_y
+        // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8).  The RY + 6 values of the thread's own
+        // x column are loaded once per field and serve the y stencils of all its outputs.
+        T ctr[RY][4], d1x[RY][4], d1y[RY][4], inpl[RY][3], ezx[RY][3];
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
-            const T* q = sp + f * FIELD;
-            ctr[f] = q[0];
-            if constexpr (TM) {
-                const uint2 u = *reinterpret_cast<const uint2*>(&ctr[f]);
-                const uint32_t r2[2] = {u.x, u.y};
-                tmem_st<2>(tdl + TWIN + f * 16 + n8 * 2, r2);
-            } else {
-                st.win[f][n8] = ctr[f];
-            }
-            const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
-            const T yp1 = q[PXS], ym1 = q[-PXS], yp2 = q[2 * PXS], ym2 = q[-2 * PXS], yp3 = q[3 * PXS], ym3 = q[-3 * PXS];
-            const T dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
-            const T dy1 = yp1 - ym1, dy2 = yp2 - ym2, dy3 = yp3 - ym3;
-            const T* a = f == 0 ? c.ar : c.au;
-            d1x[f] = fma_(a[2], dx3, fma_(a[1], dx2, a[0] * dx1));
-            d1y[f] = fma_(a[2], dy3, fma_(a[1], dy2, a[0] * dy1));
-            if (f > 0) {
-                const T sx1 = xp1 + xm1, sx2 = xp2 + xm2, sx3 = xp3 + xm3;
-                const T sy1 = yp1 + ym1, sy2 = yp2 + ym2, sy3 = yp3 + ym3;
-                const T* bx = f == 1 ? c.lq : c.lo;  // d_xx u_x and d_yy u_y carry 4nu/3 on the 55-point path
-                const T* by = f == 2 ? c.lq : c.lo;
-                T v = c.cxy[f - 1] * ctr[f];
-                v = fma_(bx[1], sx1, v);
-                v = fma_(by[1], sy1, v);
-                v = fma_(bx[2], sx2, v);
-                v = fma_(by[2], sy2, v);
-                v = fma_(bx[3], sx3, v);
-                v = fma_(by[3], sy3, v);
-                if (PATH55 && (f == 1 || f == 2)) {  // Eq. 8 in the xy plane: d_xy u_x -> rhs_y, d_xy u_y -> rhs_x
-                    const T q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
-                    const T q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
-                    const T q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
-                    const T dq = fma_(c.mq[2], q3, fma_(c.mq[1], q2, c.mq[0] * q1));
-                    if (f == 1) { inpl[0] = v; inpl[1] = dq; } else { inpl[1] += v; inpl[0] += dq; }
+            const T* q0 = sp + f * FIELD;
+            T yv[RY + 2 * R];
+#pragma unroll
+            for (int i = 0; i < RY + 2 * R; ++i) yv[i] = q0[(i - R) * PXS];
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                const T* q = q0 + r * PXS;
+                ctr[r][f] = yv[r + R];
+                if constexpr (TM) {
+                    const uint2 u = *reinterpret_cast<const uint2*>(&ctr[r][f]);
+                    const uint32_t r2[2] = {u.x, u.y};
+                    tmem_st<2>(tdl + r * TBLOCK + TWIN + f * 16 + n8 * 2, r2);
                 } else {
-                    inpl[f - 1] = v;
+                    st[r].win[f][n8] = ctr[r][f];
                 }
-            }
-            if (PATH55) {
-                if (f == 1) { ez[0] = dx1; ez[1] = dx2; ez[2] = dx3; }
-                if (f == 2) { ez[0] += dy1; ez[1] += dy2; ez[2] += dy3; }
-                if (f == 3) { ex[0] = dx1; ex[1] = dx2; ex[2] = dx3; ey[0] = dy1; ey[1] = dy2; ey[2] = dy3; }
+                const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
+                const T yp1 = yv[r + R + 1], ym1 = yv[r + R - 1], yp2 = yv[r + R + 2], ym2 = yv[r + R - 2], yp3 = yv[r + R + 3], ym3 = yv[r + R - 3];
+                const T dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
+                const T dy1 = yp1 - ym1, dy2 = yp2 - ym2, dy3 = yp3 - ym3;
+                const T* a = f == 0 ? c.ar : c.au;
+                d1x[r][f] = fma_(a[2], dx3, fma_(a[1], dx2, a[0] * dx1));
+                d1y[r][f] = fma_(a[2], dy3, fma_(a[1], dy2, a[0] * dy1));
+                if (f > 0) {
+                    const T sx1 = xp1 + xm1, sx2 = xp2 + xm2, sx3 = xp3 + xm3;
+                    const T sy1 = yp1 + ym1, sy2 = yp2 + ym2, sy3 = yp3 + ym3;
+                    const T* bx = f == 1 ? c.lq : c.lo;  // d_xx u_x and d_yy u_y carry 4nu/3 on the 55-point path
+                    const T* by = f == 2 ? c.lq : c.lo;
+                    T v = c.cxy[f - 1] * ctr[r][f];
+                    v = fma_(bx[1], sx1, v);
+                    v = fma_(by[1], sy1, v);
+                    v = fma_(bx[2], sx2, v);
+                    v = fma_(by[2], sy2, v);
+                    v = fma_(bx[3], sx3, v);
+                    v = fma_(by[3], sy3, v);
+                    if (PATH55 && (f == 1 || f == 2)) {  // Eq. 8 in the xy plane: d_xy u_x -> rhs_y, d_xy u_y -> rhs_x
+                        const T q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
+                        const T q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
+                        const T q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
+                        const T dq = fma_(c.mq[2], q3, fma_(c.mq[1], q2, c.mq[0] * q1));
+                        if (f == 1) { inpl[r][0] = v; inpl[r][1] = dq; } else { inpl[r][1] += v; inpl[r][0] += dq; }
+                    } else {
+                        inpl[r][f - 1] = v;
+                    }
+                }
+                if (PATH55) {  // the differences that feed Dzx u_x + Dzy u_y -> rhs_z, Dxz u_z -> rhs_x, Dyz u_z -> rhs_y
+                    if (f == 1) { ezx[r][0] = dx1; ezx[r][1] = dx2; ezx[r][2] = dx3; }
+                    if (f == 2) {
+                        const T ez[3] = {ezx[r][0] + dy1, ezx[r][1] + dy2, ezx[r][2] + dy3};
+                        scatter<n8>(st[r].lin[2], ez, c);
+                    }
+                    if (f == 3) {
+                        const T ex[3] = {dx1, dx2, dx3}, ey[3] = {dy1, dy2, dy3};
+                        scatter<n8>(st[r].lin[0], ex, c);
+                        scatter<n8>(st[r].lin[1], ey, c);
+                    }
+                }
             }
         }
         // ---- plane t: everything of dt*rhs that needs no z derivative (Eq. 1-3); G' = dt * grad u
-        {
-            const T gx = d1x[0], gy = d1y[0], ux = ctr[1], uy = ctr[2];
-            const T Gxx = d1x[1], Gxy = d1y[1], Gyx = d1x[2], Gyy = d1y[2], Gzx = d1x[3], Gzy = d1y[3];
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            const T gx = d1x[r][0], gy = d1y[r][0], ux = ctr[r][1], uy = ctr[r][2];
+            const T Gxx = d1x[r][1], Gxy = d1y[r][1], Gyx = d1x[r][2], Gyy = d1y[r][2], Gzx = d1x[r][3], Gzy = d1y[r][3];
             const T Dh = Gxx + Gyy;
             const T ug = fma_(uy, gy, ux * gx);
             const T P0 = fma_(-c.dt, ug, -Dh);
             const T h = fma_(-c.nu23, Dh, -c.cs2dt);
             const T nsym = c.nu * (Gxy + Gyx);
             const T kx = fma_(c.nu2, Gxx, h), ky = fma_(c.nu2, Gyy, h);
-            T tx = inpl[0], ty = inpl[1], tz = inpl[2];
+            T tx = inpl[r][0], ty = inpl[r][1], tz = inpl[r][2];
             tx = fma_(-ux, Gxx, tx);
             ty = fma_(-ux, Gyx, ty);
             tx = fma_(-uy, Gxy, tx);
@@ -301,110 +329,105 @@ struct Tiled {
             tz = fma_(Gzx, fma_(c.nu, gx, -ux), tz);
             tz = fma_(Gzy, fma_(c.nu, gy, -uy), tz);
             const T pl[3] = {tx, ty, tz};
-            if (PATH55) {
-                const T* e[3] = {ex, ey, ez};
 #pragma unroll
-                for (int i = 0; i < 3; ++i) {
-                    st.lin[i][(n8 + 3) & 7] = -(c.mq[2] * e[i][2]);  // first contribution to output t+3
-                    st.lin[i][(n8 + 2) & 7] = fma_(-c.mq[1], e[i][1], st.lin[i][(n8 + 2) & 7]);
-                    st.lin[i][(n8 + 1) & 7] = fma_(-c.mq[0], e[i][0], st.lin[i][(n8 + 1) & 7]);
-                    st.lin[i][n8] += pl[i];
-                    st.lin[i][(n8 + 7) & 7] = fma_(c.mq[0], e[i][0], st.lin[i][(n8 + 7) & 7]);
-                    st.lin[i][(n8 + 6) & 7] = fma_(c.mq[1], e[i][1], st.lin[i][(n8 + 6) & 7]);
-                    st.lin[i][(n8 + 5) & 7] = fma_(c.mq[2], e[i][2], st.lin[i][(n8 + 5) & 7]);  // output t-3 is complete
-                }
-            } else {
-#pragma unroll
-                for (int i = 0; i < 3; ++i) st.lin[i][n8] = pl[i];
+            for (int i = 0; i < 3; ++i) {
+                if (PATH55)
+                    st[r].lin[i][n8] += pl[i];
+                else
+                    st[r].lin[i][n8] = pl[i];
             }
             // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of plane t -> delay-line slot t & 3
             if constexpr (TM) {
                 const T park[6] = {gx, gy, Gzx, Gzy, Dh, P0};
-                Regs6<T>::store(tdl + n4 * DLCOLS, park);
+                Regs6<T>::store(tdl + r * TBLOCK + n4 * DLCOLS, park);
             } else {
-                st.dl[0][n4] = gx;
-                st.dl[1][n4] = gy;
-                st.dl[2][n4] = Gzx;
-                st.dl[3][n4] = Gzy;
-                st.dl[4][n4] = Dh;
-                st.dl[5][n4] = P0;
+                st[r].dl[0][n4] = gx;
+                st[r].dl[1][n4] = gy;
+                st[r].dl[2][n4] = Gzx;
+                st[r].dl[3][n4] = Gzy;
+                st[r].dl[4][n4] = Dh;
+                st[r].dl[5][n4] = P0;
             }
         }
         if (!out) return;
         // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
         constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
-        T d1z[4], fc[4], del[6];
-        if constexpr (TM) {
-            // the whole window ring of a field is 16 consecutive columns: one load each; slot t of this plane may
-            // still be in flight, so it is taken from the register that holds it
-            uint32_t wr[4][16], dr[12];
-#pragma unroll
-            for (int f = 0; f < 4; ++f) tmem_ld16(tdl + TWIN + f * 16, wr[f]);
-            tmem_ld<8>(tdl + r4 * DLCOLS, dr);
-            tmem_ld<4>(tdl + r4 * DLCOLS + 8, dr + 8);
-            tmem_wait_ld();
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-#pragma unroll
-                for (int a8 = 0; a8 < 8; ++a8) {
-                    const uint2 u = make_uint2(wr[f][2 * a8], wr[f][2 * a8 + 1]);
-                    st.win[f][a8] = *reinterpret_cast<const T*>(&u);
-                }
-                st.win[f][n8] = ctr[f];
-            }
-            Regs6<T>::unpack(dr, del);
-        } else {
-#pragma unroll
-            for (int q = 0; q < 6; ++q) del[q] = st.dl[q][r4];
-        }
-#pragma unroll
-        for (int f = 0; f < 4; ++f) {
-            const T* a = f == 0 ? c.ar : c.au;
-            fc[f] = st.win[f][cz];
-            d1z[f] = fma_(a[2], st.win[f][(cz + 3) & 7] - st.win[f][(cz + 5) & 7],
-                          fma_(a[1], st.win[f][(cz + 2) & 7] - st.win[f][(cz + 6) & 7], a[0] * (st.win[f][(cz + 1) & 7] - st.win[f][(cz + 7) & 7])));
-        }
-        T lz[3];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            const T* bz = i == 2 ? c.lq : c.lo;
-            const int f = i + 1;
-            T v = fma_(bz[0], fc[f], st.lin[i][cz]);
-            v = fma_(bz[1], st.win[f][(cz + 1) & 7] + st.win[f][(cz + 7) & 7], v);
-            v = fma_(bz[2], st.win[f][(cz + 2) & 7] + st.win[f][(cz + 6) & 7], v);
-            v = fma_(bz[3], st.win[f][(cz + 3) & 7] + st.win[f][(cz + 5) & 7], v);
-            lz[i] = v;
-        }
-        const T gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
-        const T gz = d1z[0], Gxz = d1z[1], Gyz = d1z[2], Gzz = d1z[3], uz = fc[3];
-        const T divp = Dhd + Gzz;  // dt * div u
-        T Rv[4];
-        Rv[0] = fma_(-(c.dt * uz), gz, P0d - Gzz);
-        const T ngz = c.nu * gz, m23 = c.nu23 * Gzz;
-        T rx = lz[0], ry = lz[1], rz = lz[2];
-        rx = fma_(-uz, Gxz, rx);
-        ry = fma_(-uz, Gyz, ry);
-        rz = fma_(-uz, Gzz, rz);
-        rx = fma_(ngz, Gxz + Gzxd, rx);
-        ry = fma_(ngz, Gyz + Gzyd, ry);
-        rz = fma_(gz, fma_(c.nu2, Gzz, fma_(-c.nu23, divp, -c.cs2dt)), rz);
-        rx = fma_(-m23, gxd, rx);
-        ry = fma_(-m23, gyd, ry);
-        rz = fma_(c.nu * gxd, Gxz, rz);
-        rz = fma_(c.nu * gyd, Gyz, rz);
-        Rv[1] = rx;
-        Rv[2] = ry;
-        Rv[3] = rz;
-        // ---- Eq. 10; coalesced 64/128/256-byte row segments per warp straight to global memory
         const T* wsp = wsp0 + ((PH + 2) & 3) * WSTAGE;  // w ring slot of plane index p - 6
-        if (store_ok) {
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            T d1z[4], fc[4], del[6];
+            if constexpr (TM) {
+                // the whole window ring of a field is 16 consecutive columns: one load each; slot t of this plane may
+                // still be in flight, so it is taken from the register that holds it
+                uint32_t wr[4][16], dr[12];
+#pragma unroll
+                for (int f = 0; f < 4; ++f) tmem_ld16(tdl + r * TBLOCK + TWIN + f * 16, wr[f]);
+                tmem_ld<8>(tdl + r * TBLOCK + r4 * DLCOLS, dr);
+                tmem_ld<4>(tdl + r * TBLOCK + r4 * DLCOLS + 8, dr + 8);
+                tmem_wait_ld();
+#pragma unroll
+                for (int f = 0; f < 4; ++f) {
+#pragma unroll
+                    for (int a8 = 0; a8 < 8; ++a8) {
+                        const uint2 u = make_uint2(wr[f][2 * a8], wr[f][2 * a8 + 1]);
+                        st[r].win[f][a8] = *reinterpret_cast<const T*>(&u);
+                    }
+                    st[r].win[f][n8] = ctr[r][f];
+                }
+                Regs6<T>::unpack(dr, del);
+            } else {
+#pragma unroll
+                for (int q = 0; q < 6; ++q) del[q] = st[r].dl[q][r4];
+            }
+            const T(&win)[4][8] = st[r].win;
 #pragma unroll
             for (int f = 0; f < 4; ++f) {
-                const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD], Rv[f]) : Rv[f];
-                if (c.write_w) gW[f * n] = wn;
-                if (c.write_f) gF[f * fs] = fma_(c.beta, wn, fc[f]);
+                const T* a = f == 0 ? c.ar : c.au;
+                fc[f] = win[f][cz];
+                d1z[f] = fma_(a[2], win[f][(cz + 3) & 7] - win[f][(cz + 5) & 7],
+                              fma_(a[1], win[f][(cz + 2) & 7] - win[f][(cz + 6) & 7], a[0] * (win[f][(cz + 1) & 7] - win[f][(cz + 7) & 7])));
             }
-            if (!PATH55) *gD = divp;
+            T lz[3];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+                const T* bz = i == 2 ? c.lq : c.lo;
+                const int f = i + 1;
+                T v = fma_(bz[0], fc[f], st[r].lin[i][cz]);
+                v = fma_(bz[1], win[f][(cz + 1) & 7] + win[f][(cz + 7) & 7], v);
+                v = fma_(bz[2], win[f][(cz + 2) & 7] + win[f][(cz + 6) & 7], v);
+                v = fma_(bz[3], win[f][(cz + 3) & 7] + win[f][(cz + 5) & 7], v);
+                lz[i] = v;
+            }
+            const T gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
+            const T gz = d1z[0], Gxz = d1z[1], Gyz = d1z[2], Gzz = d1z[3], uz = fc[3];
+            const T divp = Dhd + Gzz;  // dt * div u
+            T Rv[4];
+            Rv[0] = fma_(-(c.dt * uz), gz, P0d - Gzz);
+            const T ngz = c.nu * gz, m23 = c.nu23 * Gzz;
+            T rx = lz[0], ry = lz[1], rz = lz[2];
+            rx = fma_(-uz, Gxz, rx);
+            ry = fma_(-uz, Gyz, ry);
+            rz = fma_(-uz, Gzz, rz);
+            rx = fma_(ngz, Gxz + Gzxd, rx);
+            ry = fma_(ngz, Gyz + Gzyd, ry);
+            rz = fma_(gz, fma_(c.nu2, Gzz, fma_(-c.nu23, divp, -c.cs2dt)), rz);
+            rx = fma_(-m23, gxd, rx);
+            ry = fma_(-m23, gyd, ry);
+            rz = fma_(c.nu * gxd, Gxz, rz);
+            rz = fma_(c.nu * gyd, Gyz, rz);
+            Rv[1] = rx;
+            Rv[2] = ry;
+            Rv[3] = rz;
+            // ---- Eq. 10; coalesced row segments per warp straight to global memory
+            if (ok[r]) {
+#pragma unroll
+                for (int f = 0; f < 4; ++f) {
+                    const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD + r * TX], Rv[f]) : Rv[f];
+                    if (c.write_w) gW[f * n + r * pw] = wn;
+                    if (c.write_f) gF[f * fs + r * pf] = fma_(c.beta, wn, fc[f]);
+                }
+                if (!PATH55) gD[r * pf] = divp;
+            }
         }
     }
 
@@ -427,7 +450,7 @@ struct Tiled {
             ze = min(zs + sc.zc, g.nz);
         }
         if (zs >= ze) return;  // empty chunk (rounding); the whole CTA leaves before any barrier
-        const int X0 = (tile % sc.ntx) * TX, Y0 = (tile / sc.ntx) * TY;
+        const int X0 = (tile % sc.ntx) * TX, Y0 = (tile / sc.ntx) * TH;
         const int np = ze - zs + 2 * R;  // staged planes t = zs-3 .. ze+2
         constexpr int L = Scalar<T>::lanes;
         // TMA box origin; the tensor maps count scalars along x, a value is L of them
@@ -459,34 +482,40 @@ struct Tiled {
             __syncthreads();
         }
         // a warp reaches the 32 lanes of its quadrant (warp % 4); warps that share a quadrant use different columns
-        const uint32_t tdl = tmem_base + ((uint32_t)(((tid >> 5) & 3) * 32) << 16) + (uint32_t)((tid >> 7) * TBLOCK);
+        const uint32_t tdl = tmem_base + ((uint32_t)(((tid >> 5) & 3) * 32) << 16) + (uint32_t)((tid >> 7) * RY * TBLOCK);
         if (producer) {
             for (int i = 0; i < NS && i < np; ++i) {
                 mbar_expect_tx(a_full + 8 * i, kStageBytes);
                 tma_load_4d(a_sm + i * kStageBytes, &m.f_in, a_full + 8 * i, bx, by, bz + i, 0);
             }
         }
-        const T* sp0 = sm + (ty + R) * PXS + (tx + 4);
-        const T* wsp0 = smw + ty * TX + tx;
-        // this thread's cell of output plane zs in the dense (w) and padded (F, div) arrays; advanced plane by plane
-        const int ci = X0 + tx, cj = Y0 + ty;
-        const bool store_ok = ci < g.nx && cj < g.ny;
+        const T* sp0 = sm + (ty * RY + R) * PXS + (tx + 4);
+        const T* wsp0 = smw + ty * RY * TX + tx;
+        // this thread's first cell of output plane zs in the dense (w) and padded (F, div) arrays; advanced plane by plane
+        const int ci = X0 + tx, cj = Y0 + ty * RY;
+        bool ok[RY];
+#pragma unroll
+        for (int r = 0; r < RY; ++r) ok[r] = ci < g.nx && cj + r < g.ny;
+        const bool store_ok = ok[0];
         const long long plane_w = (long long)g.nx * g.ny, plane_f = (long long)g.px * g.py;
         long long ow = ci + (long long)g.nx * (cj + (long long)g.ny * zs);
         long long of = (ci + g.gx) + (long long)g.px * ((cj + g.gy) + (long long)g.py * (zs + g.gz));
         if (!store_ok) { ow = 0; of = 0; }
-        State st;
+        State st[RY];
 #pragma unroll
-        for (int a = 0; a < 8; ++a) {
+        for (int r = 0; r < RY; ++r) {
 #pragma unroll
-            for (int f = 0; f < 4; ++f) st.win[f][a] = T(0);
+            for (int a = 0; a < 8; ++a) {
 #pragma unroll
-            for (int q = 0; q < 3; ++q) st.lin[q][a] = T(0);
+                for (int f = 0; f < 4; ++f) st[r].win[f][a] = T(0);
+#pragma unroll
+                for (int q = 0; q < 3; ++q) st[r].lin[q][a] = T(0);
+            }
+#pragma unroll
+            for (int q = 0; q < 6; ++q)
+#pragma unroll
+                for (int a = 0; a < 4; ++a) st[r].dl[q][a] = T(0);
         }
-#pragma unroll
-        for (int q = 0; q < 6; ++q)
-#pragma unroll
-            for (int a = 0; a < 4; ++a) st.dl[q][a] = T(0);
 
         for (int pb = 0; pb < np; pb += 8) {
 #pragma unroll
@@ -497,7 +526,7 @@ struct Tiled {
                     if constexpr (TM) tmem_wait_st();  // what the previous planes parked in tensor memory is in place
                     mbar_wait(a_full + 8 * (ph & (NS - 1)), (uint32_t)((p >> LNS) & 1));
                     if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
-#define FD6_STEP(K) step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, store_ok)
+#define FD6_STEP(K) step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, g.px, g.nx, ok)
                     switch (ph) {  // ph is a compile-time constant after unrolling
                         case 0: FD6_STEP(0); break;
                         case 1: FD6_STEP(1); break;
@@ -545,27 +574,29 @@ struct Tiled {
     }
 };
 
-template <class T, bool PATH55, int TX, int TY, int NS>
+template <class T, bool PATH55, int TX, int TY, int NS, int RY>
 __global__ void __launch_bounds__(TX* TY, 1)
     k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, const Sched sc, T* __restrict__ Fout,
                  T* __restrict__ W, T* __restrict__ Div) {
-    Tiled<T, PATH55, TX, TY, NS>::run(m, g, c, sc, Fout, W, Div);
+    Tiled<T, PATH55, TX, TY, NS, RY>::run(m, g, c, sc, Fout, W, Div);
 }
 
-// Tile shape per value type (registers per thread bound the CTA size).
+// Tile shape per value type (registers per thread bound the CTA size).  RY = 2 (two vertically
+// adjacent outputs per thread, 13 % fewer shared-memory loads per value, 217 registers, 8 warps) is bit-identical
+// and was measured 6 % slower than RY = 1 with 12 warps for the paired fused kernel, equal for pass 1.
 template <class T>
 struct TileShape;
 template <>
 struct TileShape<float> {
-    static constexpr int TX = 64, TY = 8, NS = 8;  // 16 warps x 128 registers, state in registers
+    static constexpr int TX = 64, TY = 8, NS = 8, RY = 1;  // 16 warps x 128 registers, state in registers
 };
 template <>
 struct TileShape<double> {
-    static constexpr int TX = 32, TY = 8, NS = 4;  // 8 warps; window and delay line in tensor memory (12 warps measured slower: DFMA-bound)
+    static constexpr int TX = 32, TY = 8, NS = 4, RY = 1;  // 8 warps; window and delay line in tensor memory (12 warps measured slower: DFMA-bound)
 };
 template <>
 struct TileShape<V2> {
-    static constexpr int TX = 32, TY = 12, NS = 4;  // 12 warps x <= 168 registers: window and delay line in tensor memory
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x <= 168 registers: window and delay line in tensor memory
 };
 
 // ---- host side -------------------------------------------------------------------------------------------
@@ -655,20 +686,20 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
 template <class T>
 static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
     ts.ready = false;
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS;
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
     void* F[2] = {F0, F1};
     int rc = 0;
     for (int cur = 0; cur < 2 && rc == 0; ++cur) {
         Maps& m = ts.maps[cur];
-        rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TY + 2 * R, 4);
-        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY, 4);
+        rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TY * RY + 2 * R, 4);
+        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY * RY, 4);
     }
     if (rc) return rc;
-    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Tiled<T, true, TX, TY, NS>::SMEM);
+    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)Tiled<T, true, TX, TY, NS, RY>::SMEM);
     if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Tiled<T, false, TX, TY, NS>::SMEM);
+        e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)Tiled<T, false, TX, TY, NS, RY>::SMEM);
     if (e != cudaSuccess) {
         snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
         cudaGetLastError();
@@ -678,7 +709,7 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
-    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TY - 1) / TY, g.nz, ts.sm_count, &ts.items);
+    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TY * RY - 1) / (TY * RY), g.nz, ts.sm_count, &ts.items);
     ts.ready = true;
     return 0;
 }
@@ -726,12 +757,12 @@ static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
 template <class T>
 static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
                              cudaStream_t stream) {
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS;
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
     dim3 block(TX, TY, 1), grid(ts.items, 1, 1);
     if (path55)
-        k_tiled_main<T, true, TX, TY, NS><<<grid, block, Tiled<T, true, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
+        k_tiled_main<T, true, TX, TY, NS, RY><<<grid, block, Tiled<T, true, TX, TY, NS, RY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
     else
-        k_tiled_main<T, false, TX, TY, NS><<<grid, block, Tiled<T, false, TX, TY, NS>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
+        k_tiled_main<T, false, TX, TY, NS, RY><<<grid, block, Tiled<T, false, TX, TY, NS, RY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 
