@@ -58,12 +58,11 @@ enum {
 enum {
     FD_K_PACK = 0,    /* dense -> padded interior */
     FD_K_UNPACK = 1,  /* padded interior -> dense                         (a0)             */
-    FD_K_HALO_X = 2,  /* periodic ghost fill, x faces                     (a1, a7)         */
-    FD_K_HALO_YZ = 3, /* periodic ghost fill, y/z faces and all edges     (a1, a7)         */
-    FD_K_FUSED55 = 4, /* Eq. 6-8 + Eq. 1-3 + Eq. 10, one pass             (a2-a4)          */
-    FD_K_PASS1 = 5,   /* 19-pt pass 1: div u, partial update Eq. 14-16    (a6)             */
-    FD_K_PASS2 = 6,   /* 19-pt pass 2: grad div by Eq. 6, Eq. 17-18       (a8)             */
-    FD_K_COUNT = 7
+    FD_K_HALO = 2,    /* periodic ghost fill: all faces and edges         (a1, a7)         */
+    FD_K_FUSED55 = 3, /* Eq. 6-8 + Eq. 1-3 + Eq. 10, one pass             (a2-a4)          */
+    FD_K_PASS1 = 4,   /* 19-pt pass 1: div u, partial update Eq. 14-16    (a6)             */
+    FD_K_PASS2 = 5,   /* 19-pt pass 2: grad div by Eq. 6, Eq. 17-18       (a8)             */
+    FD_K_COUNT = 6
 };
 
 /* Device-memory hooks.  alloc returns a device pointer aligned to >= 256 bytes or NULL; `stream` is the

@@ -245,16 +245,11 @@ static bool pair_ok(const fd_ctx* c) { return c->dtype == FD_F32 && c->nz % 2 ==
 template <class T>
 static int launch_halo(fd_ctx* c, T* F, int nfields) {
     const Geom& g = c->g;
-    {
-        LaunchScope ls(c, FD_K_HALO_X);
-        long long threads = 2LL * g.ny * g.nz * nfields;
-        k_halo_x<T><<<(unsigned)((threads + 127) / 128), 128, 0, c->stream>>>(F, g, nfields);
-    }
-    {
-        LaunchScope ls(c, FD_K_HALO_YZ);
-        dim3 grid(2 * R * g.py + 2 * R * g.nz, nfields);
-        k_halo_yz<T><<<grid, 128, 0, c->stream>>>(F, g);
-    }
+    LaunchScope ls(c, FD_K_HALO);
+    const int yz_rows = 2 * R * g.py + 2 * R * g.nz;
+    const long long xthreads = 2LL * g.ny * g.nz * nfields;
+    const long long blocks = (long long)nfields * yz_rows + (xthreads + 127) / 128;
+    k_halo<T><<<(unsigned)blocks, 128, 0, c->stream>>>(F, g, nfields, yz_rows);
     FD_CUDA(cudaGetLastError());
     return FD_OK;
 }

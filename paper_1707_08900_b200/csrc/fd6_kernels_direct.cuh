@@ -54,17 +54,48 @@ __global__ void __launch_bounds__(128)
 // ------------------------------------------------------------------------------------------------
 // a1 / a7  periodic halo fill, radius 3 (Alg. 2/3 "Compute boundary conditions").
 //   (T = V2: the stored grid has nz/2 planes and z-periodicity swaps the halves of a pair, see zwrap.)
-//   k_halo_x : every interior row (j,k) copies one 32-byte sector to each x ghost pad.   thread per (row, side, field)
-//   k_halo_yz: every ghost ROW (j or k outside the domain) is the x-extended copy of the interior row it
-//              wraps to; run after k_halo_x so edge ghosts (two coordinates outside, needed by the Eq. 8
-//              diagonals) come along.  Corner ghosts are filled too (never read).
+//   One kernel, every ghost value read straight from the interior (no ordering between faces):
+//   blocks [0, nfields * yz_rows): one ghost ROW each (j or k outside the domain) = the x-extended copy of the
+//       interior row it wraps to, its own 2R x ghosts taken from the far end of that row; this also fills the
+//       edge ghosts (two coordinates outside) the Eq. 8 diagonals read, and the corners (never read);
+//   remaining blocks: the x ghosts of the interior rows, one thread per (row, side): the x ghost pad is exactly one
+//       32-byte sector (gx values) and rows are 32-byte aligned, so a side is one aligned sector copy — the low pad
+//       [0, gx) takes the last gx interior values, the high pad the first gx (only R of them are ever read).
 // ------------------------------------------------------------------------------------------------
 template <class T>
-__global__ void __launch_bounds__(128) k_halo_x(T* __restrict__ F, Geom g, int nfields) {
-    // One thread per (row, side).  The x ghost pad is exactly one 32-byte sector (gx values) and rows are 32-byte
-    // aligned, so a side is one aligned sector copy: the low pad [0, gx) takes the last gx interior values, the high
-    // pad [gx+nx, 2gx+nx) the first gx (only the R values next to the interior are ever read).
-    long long t = (long long)blockIdx.x * 128 + threadIdx.x;
+__global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfields, int yz_rows) {
+    if ((int)blockIdx.x < nfields * yz_rows) {
+        // ghost rows: first the 2R ghost z-planes (py rows each), then for every interior plane its 2R ghost y-rows
+        const int q = blockIdx.x / yz_rows;
+        int b = blockIdx.x - q * yz_rows, jj, kk;
+        const int zrows = 2 * R * g.py;
+        if (b < zrows) {
+            int zp = b / g.py;
+            jj = b - zp * g.py;
+            kk = zp < R ? zp + (g.gz - R) : g.gz + g.nz + (zp - R);
+        } else {
+            b -= zrows;
+            int k = b / (2 * R), yr = b - k * (2 * R);
+            kk = k + g.gz;
+            jj = yr < R ? yr + (g.gy - R) : g.gy + g.ny + (yr - R);
+        }
+        int js = jj - g.gy, ks = kk - g.gz;  // wrap to the interior row (n >= R: one correction suffices)
+        js += js < 0 ? g.ny : 0;
+        js -= js >= g.ny ? g.ny : 0;
+        const bool zw = ks < 0 || ks >= g.nz;  // paired layout: crossing the z boundary swaps the two halves
+        ks += ks < 0 ? g.nz : 0;
+        ks -= ks >= g.nz ? g.nz : 0;
+        T* base = F + q * g.fs;
+        T* dst = base + (long long)g.px * (jj + (long long)g.py * kk) + (g.gx - R);
+        const T* src = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz)) + (g.gx - R);
+        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) {
+            const int xs = x < R ? x + g.nx : (x >= g.nx + R ? x - g.nx : x);
+            const T v = src[xs];
+            dst[x] = zw ? zwrap<T>(v) : v;
+        }
+        return;
+    }
+    long long t = (long long)(blockIdx.x - nfields * yz_rows) * 128 + threadIdx.x;
     const int side = (int)(t & 1);
     t >>= 1;
     long long rows = (long long)g.ny * g.nz;
@@ -78,38 +109,6 @@ __global__ void __launch_bounds__(128) k_halo_x(T* __restrict__ F, Geom g, int n
     const uint4 a = src[0], b = src[1];
     dst[0] = a;
     dst[1] = b;
-}
-
-template <class T>
-__global__ void __launch_bounds__(128) k_halo_yz(T* __restrict__ F, Geom g) {
-    // blockIdx.x enumerates ghost rows: first the 2R ghost z-planes (py rows each), then for every
-    // interior plane its 2R ghost y-rows.  blockIdx.y = field.
-    int b = blockIdx.x, jj, kk;
-    const int zrows = 2 * R * g.py;
-    if (b < zrows) {
-        int zp = b / g.py;
-        jj = b - zp * g.py;
-        kk = zp < R ? zp + (g.gz - R) : g.gz + g.nz + (zp - R);
-    } else {
-        b -= zrows;
-        int k = b / (2 * R), yr = b - k * (2 * R);
-        kk = k + g.gz;
-        jj = yr < R ? yr + (g.gy - R) : g.gy + g.ny + (yr - R);
-    }
-    int js = jj - g.gy, ks = kk - g.gz;  // wrap to the interior row (n >= R: one correction suffices)
-    js += js < 0 ? g.ny : 0;
-    js -= js >= g.ny ? g.ny : 0;
-    const bool zw = ks < 0 || ks >= g.nz;  // paired layout: crossing the z boundary swaps the two halves
-    ks += ks < 0 ? g.nz : 0;
-    ks -= ks >= g.nz ? g.nz : 0;
-    T* base = F + blockIdx.y * g.fs;
-    T* dst = base + (long long)g.px * (jj + (long long)g.py * kk) + (g.gx - R);
-    const T* src = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz)) + (g.gx - R);
-    if (zw) {
-        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = zwrap<T>(src[x]);
-    } else {
-        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) dst[x] = src[x];
-    }
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -18,8 +18,8 @@ FD_PATH_55, FD_PATH_19 = 0, 1
 FD_HOST, FD_DEVICE = 0, 1
 FD_OK, FD_EINVAL, FD_ENOMEM, FD_ECUDA, FD_EUNSUPPORTED = 0, 1, 2, 3, 4
 FD_VARIANT_AUTO, FD_VARIANT_DIRECT, FD_VARIANT_TILED, FD_VARIANT_PAIRED = 0, 1, 2, 3
-FD_K_PACK, FD_K_UNPACK, FD_K_HALO_X, FD_K_HALO_YZ, FD_K_FUSED55, FD_K_PASS1, FD_K_PASS2, FD_K_COUNT = range(8)
-KERNEL_NAMES = ["pack", "unpack", "halo_x", "halo_yz", "fused55", "pass1_19", "pass2_19"]
+FD_K_PACK, FD_K_UNPACK, FD_K_HALO, FD_K_FUSED55, FD_K_PASS1, FD_K_PASS2, FD_K_COUNT = range(7)
+KERNEL_NAMES = ["pack", "unpack", "halo", "fused55", "pass1_19", "pass2_19"]
 
 EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
