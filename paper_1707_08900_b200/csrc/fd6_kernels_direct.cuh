@@ -86,12 +86,34 @@ __global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfi
         ks += ks < 0 ? g.nz : 0;
         ks -= ks >= g.nz ? g.nz : 0;
         T* base = F + q * g.fs;
-        T* dst = base + (long long)g.px * (jj + (long long)g.py * kk) + (g.gx - R);
-        const T* src = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz)) + (g.gx - R);
-        for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) {
-            const int xs = x < R ? x + g.nx : (x >= g.nx + R ? x - g.nx : x);
-            const T v = src[xs];
-            dst[x] = zw ? zwrap<T>(v) : v;
+        T* drow = base + (long long)g.px * (jj + (long long)g.py * kk);
+        const T* srow = base + (long long)g.px * ((js + g.gy) + (long long)g.py * (ks + g.gz));
+        if (g.nx % g.gx == 0) {
+            // whole 32-byte sectors (gx values): sector 0 is the low pad, the last one the high pad
+            constexpr int VPS = (int)(32 / sizeof(T));  // == g.gx
+            const int nsec = g.nx / VPS + 2;
+            for (int sct = threadIdx.x; sct < nsec; sct += 128) {
+                const int ssrc = sct == 0 ? nsec - 2 : (sct == nsec - 1 ? 1 : sct);
+                union { uint4 u[2]; T v[VPS]; } buf;
+                const uint4* sp = reinterpret_cast<const uint4*>(srow + ssrc * VPS);
+                buf.u[0] = sp[0];
+                buf.u[1] = sp[1];
+                if (zw) {
+#pragma unroll
+                    for (int e = 0; e < VPS; ++e) buf.v[e] = zwrap<T>(buf.v[e]);
+                }
+                uint4* dp = reinterpret_cast<uint4*>(drow + sct * VPS);
+                dp[0] = buf.u[0];
+                dp[1] = buf.u[1];
+            }
+        } else {
+            T* dst = drow + (g.gx - R);
+            const T* src = srow + (g.gx - R);
+            for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) {
+                const int xs = x < R ? x + g.nx : (x >= g.nx + R ? x - g.nx : x);
+                const T v = src[xs];
+                dst[x] = zw ? zwrap<T>(v) : v;
+            }
         }
         return;
     }
