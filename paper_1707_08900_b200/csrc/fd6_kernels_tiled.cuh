@@ -592,7 +592,7 @@ struct TileShape<float> {
 };
 template <>
 struct TileShape<double> {
-    static constexpr int TX = 32, TY = 8, NS = 4, RY = 1;  // 8 warps; window and delay line in tensor memory (12 warps measured slower: DFMA-bound)
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x 168 registers: window and delay line in tensor memory
 };
 template <>
 struct TileShape<V2> {

@@ -108,7 +108,7 @@ def test_c1_one_step_and_rhs_full_grid_fp64(mods, path, variant):
 
 
 # ------------------------------------------- ragged sizes spanning several tiles plus a tail
-@pytest.mark.parametrize("shape", [(40, 13, 9), (8, 8, 8), (132, 70, 20), (72, 33, 41)])
+@pytest.mark.parametrize("shape", [(40, 13, 9), (8, 8, 8), (132, 70, 20), (72, 33, 41), (44, 9, 11)])
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
 @pytest.mark.parametrize("path", [0, 1])
 @pytest.mark.parametrize("variant", [1, 2, 3])
