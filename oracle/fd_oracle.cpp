@@ -23,6 +23,7 @@
 // The only parallelism is one `#pragma omp parallel for` over k-planes; every cell
 // is independent inside a sweep, so threading does not change any result bit.
 
+#include <cmath>
 #include <cstddef>
 #include <cstdint>
 #include <vector>
@@ -161,7 +162,31 @@ inline void grad_div_55(const T* const F[4], const Dims& d, int i, int j, int k,
     }
 }
 
-// Eq. 1-3 assembled (O7).  R[0] continuity, R[1..3] momentum; f = 0 (G8).
+// ---------------------------------------------------------------------------------
+// O11  Forcing term of Eq. 2:  f(x) = Re{ N f_k exp(i k.x + i phi) }            (Eq. 24)
+//   N = f0 cs sqrt(|k| cs / dt),   f_k = (k x e) / sqrt(|k|^2 - (k.e)^2)                            (Eq. 25)
+// f_k is real, so f = N f_k cos(k.x + phi).  One (k, e, phi) is frozen over a step ("picked randomly at
+// every timestep"); x = (i, j, k) dx, the origin is cell 0 shifted by `origin` cells (windowed runs).  f0 = 0: off,
+// the paper's performance runs (G8).  Evaluated in double whatever T is.
+// ---------------------------------------------------------------------------------
+struct Forcing {
+    double k[3] = {0, 0, 0}, e[3] = {0, 0, 0}, phi = 0, f0 = 0, dt = 1, origin[3] = {0, 0, 0};
+};
+static Forcing g_forcing;
+
+inline void forcing_at(const Forcing& fo, double cs, double dx, int i, int j, int k, double f[3]) {
+    const double* kv = fo.k;
+    const double k2 = kv[0] * kv[0] + kv[1] * kv[1] + kv[2] * kv[2];
+    const double ke = kv[0] * fo.e[0] + kv[1] * fo.e[1] + kv[2] * fo.e[2];
+    const double N = fo.f0 * cs * std::sqrt(std::sqrt(k2) * cs / fo.dt);
+    const double den = std::sqrt(k2 - ke * ke);
+    const double cr[3] = {kv[1] * fo.e[2] - kv[2] * fo.e[1], kv[2] * fo.e[0] - kv[0] * fo.e[2], kv[0] * fo.e[1] - kv[1] * fo.e[0]};
+    const double x[3] = {(i + fo.origin[0]) * dx, (j + fo.origin[1]) * dx, (k + fo.origin[2]) * dx};
+    const double c = std::cos(kv[0] * x[0] + kv[1] * x[1] + kv[2] * x[2] + fo.phi);
+    for (int a = 0; a < 3; ++a) f[a] = N * (cr[a] / den) * c;
+}
+
+// Eq. 1-3 assembled (O7).  R[0] continuity, R[1..3] momentum; the forcing f of Eq. 2 is added by the callers (O11).
 template <class T>
 inline void assemble_rhs(const T u[3], const CellDerivs<T>& c, const T Q[3], bool include_Q, T nu, T cs, T R[4]) {
     // Eq. 1:  d_t ln rho = -u . grad ln rho - div u
@@ -217,6 +242,11 @@ void rhs_full(int path, const Dims& d, T dx, T nu, T cs, const T* const F[4], T*
                 T u[3] = {F[1][p], F[2][p], F[3][p]};
                 T r[4];
                 assemble_rhs(u, c, Q, true, nu, cs, r);
+                if (g_forcing.f0 != 0) {  // + f (Eq. 2, Eq. 24)
+                    double f[3];
+                    forcing_at(g_forcing, (double)cs, (double)dx, i, j, k, f);
+                    for (int a = 0; a < 3; ++a) r[1 + a] += T(f[a]);
+                }
                 for (int q = 0; q < 4; ++q) R[q][p] = r[q];
             }
 }
@@ -273,6 +303,11 @@ void rk3_steps(int path, const Dims& d, T dx, T nu, T cs, T dt, int nsteps, T* c
                         T u[3] = {Fc[1][p], Fc[2][p], Fc[3][p]};
                         T r[4];
                         assemble_rhs(u, c, Q, path == PATH_55, nu, cs, r);
+                        if (g_forcing.f0 != 0) {  // + f (Eq. 2, Eq. 24): the same frozen f on all three substeps
+                            double f[3];
+                            forcing_at(g_forcing, (double)cs, (double)dx, i, j, k, f);
+                            for (int a = 0; a < 3; ++a) r[1 + a] += T(f[a]);
+                        }
                         for (int q = 0; q < 4; ++q) rk_update(s, dt, r[q], Fc[q][p], W[q][p], out[q][p]);
                     }
             if (path == PATH_19) {
@@ -354,6 +389,26 @@ void fdo_set_num_threads(int n) {
 #else
     (void)n;
 #endif
+}
+
+// Forcing of every later fdo_rhs_* / fdo_rk3_step_* call (O11); f0 = 0 switches it off.  dt is the step size N is
+// formed with (Eq. 25); origin = cell offset of array index 0 (windowed runs).  1: bad arguments (k parallel to e, dt <= 0).
+int fdo_set_forcing(const double k[3], const double e[3], double phi, double f0, double dt, const double origin[3]) {
+    Forcing fo;
+    if (f0 != 0) {
+        const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2], ke = k[0] * e[0] + k[1] * e[1] + k[2] * e[2];
+        if (!(dt > 0) || !(k2 - ke * ke > 0)) return 1;
+        for (int a = 0; a < 3; ++a) {
+            fo.k[a] = k[a];
+            fo.e[a] = e[a];
+            fo.origin[a] = origin ? origin[a] : 0.0;
+        }
+        fo.phi = phi;
+        fo.f0 = f0;
+        fo.dt = dt;
+    }
+    g_forcing = fo;
+    return 0;
 }
 
 // Stencils on caller-gathered values (non-periodic use: polynomial exactness, pin P1).

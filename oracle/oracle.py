@@ -42,6 +42,7 @@ def lib():
         _lib.fdo_rk3_step_f64.argtypes = [i, i, i, i, d, d, d, d, i] + [pd] * 8
         _lib.fdo_rk3_step_f32.argtypes = [i, i, i, i, d, d, d, d, i] + [pf] * 8
         _lib.fdo_rk3_linear.argtypes = [d, d, d, i, pd, pd]
+        _lib.fdo_set_forcing.argtypes = [pd, pd, d, d, d, pd]
     return _lib
 
 
@@ -93,32 +94,58 @@ def deriv(f, kind, a, b=-1, dx=1.0):
     return out
 
 
+class forcing:
+    """Context manager: the forcing term of Eq. 2 (Eq. 24-25) for the oracle calls inside it.
+    spec = dict(k=(kx,ky,kz), e=(ex,ey,ez), phi=..., f0=..., dt=...) or None; origin = cell offset of index 0."""
+
+    def __init__(self, spec, origin=(0, 0, 0)):
+        self.spec, self.origin = spec, origin
+
+    def __enter__(self):
+        if self.spec is not None:
+            sp = self.spec
+            rc = lib().fdo_set_forcing(_p(_vec(sp["k"], 3)), _p(_vec(sp["e"], 3)), float(sp["phi"]), float(sp["f0"]),
+                                       float(sp["dt"]), _p(_vec(self.origin, 3)))
+            if rc:
+                raise ValueError("fdo_set_forcing: bad arguments")
+        return self
+
+    def __exit__(self, *a):
+        z = _vec((0, 0, 0), 3)
+        lib().fdo_set_forcing(_p(z), _p(z), 0.0, 0.0, 1.0, _p(z))
+
+
 def _state(F, dtype):
     F = np.ascontiguousarray(F, dtype=dtype)
     assert F.ndim == 4 and F.shape[0] == 4, "state must have shape (4, nz, ny, nx)"
     return F
 
 
-def rhs(F, dx, nu, cs, path=PATH_55, dtype=np.float64):
-    """Full right-hand side (Eq. 1-3, including nu/3 grad div u) of state F; returns (4,nz,ny,nx)."""
+def rhs(F, dx, nu, cs, path=PATH_55, dtype=np.float64, force=None):
+    """Full right-hand side (Eq. 1-3, including nu/3 grad div u, plus the forcing `force` if given) of state F;
+    returns (4,nz,ny,nx)."""
     F = _state(F, dtype)
     _, nz, ny, nx = F.shape
     R = np.empty_like(F)
     fn = lib().fdo_rhs_f64 if dtype == np.float64 else lib().fdo_rhs_f32
-    rc = fn(path, nx, ny, nz, float(dx), float(nu), float(cs), *[_p(F[q]) for q in range(4)], *[_p(R[q]) for q in range(4)])
+    with forcing(force):
+        rc = fn(path, nx, ny, nz, float(dx), float(nu), float(cs), *[_p(F[q]) for q in range(4)], *[_p(R[q]) for q in range(4)])
     if rc:
         raise ValueError("fdo_rhs: bad arguments")
     return R
 
 
-def rk3_step(F, dx, nu, cs, dt, nsteps=1, path=PATH_55, dtype=np.float64, W=None, return_w=False):
-    """nsteps full 2N-RK3 steps (Eq. 10, Alg. 2 / Alg. 3). Returns the new state (a copy)."""
+def rk3_step(F, dx, nu, cs, dt, nsteps=1, path=PATH_55, dtype=np.float64, W=None, return_w=False, force=None,
+             origin=(0, 0, 0)):
+    """nsteps full 2N-RK3 steps (Eq. 10, Alg. 2 / Alg. 3), with the frozen forcing `force` if given.
+    Returns the new state (a copy)."""
     F = _state(F, dtype).copy()
     _, nz, ny, nx = F.shape
     W = np.zeros_like(F) if W is None else _state(W, dtype).copy()
     fn = lib().fdo_rk3_step_f64 if dtype == np.float64 else lib().fdo_rk3_step_f32
-    rc = fn(path, nx, ny, nz, float(dx), float(nu), float(cs), float(dt), int(nsteps),
-            *[_p(F[q]) for q in range(4)], *[_p(W[q]) for q in range(4)])
+    with forcing(force, origin):
+        rc = fn(path, nx, ny, nz, float(dx), float(nu), float(cs), float(dt), int(nsteps),
+                *[_p(F[q]) for q in range(4)], *[_p(W[q]) for q in range(4)])
     if rc:
         raise ValueError("fdo_rk3_step: bad arguments")
     return (F, W) if return_w else F

@@ -553,3 +553,93 @@ def test_p12_float_instantiation_tracks_double():
     b = O.rk3_step(F32, dx, cfg.nu, cfg.cs, 0.1 * dx, 1, P55, dtype=np.float32)
     assert b.dtype == np.float32
     assert relinf(b.astype(np.float64), a) < 2e-6
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# P13  forcing term of Eq. 2 (Eq. 24-25, oracle step O11)
+def _forcing_expected(spec, cs):
+    """N and the unit vector f_k of Eq. 25, from vector algebra only."""
+    k, e = np.asarray(spec["k"], float), np.asarray(spec["e"], float)
+    N = spec["f0"] * cs * math.sqrt(np.linalg.norm(k) * cs / spec["dt"])
+    fk = np.cross(k, e)
+    return N, fk / np.linalg.norm(fk)  # |k x e| = sqrt(|k|^2 |e|^2 - (k.e)^2) for a unit e (Lagrange's identity)
+
+
+def test_p13_forcing_field_is_one_transverse_fourier_mode_of_amplitude_n():
+    n, cs = 16, 1.3
+    dx = TWO_PI / n
+    e = np.array([0.3, -0.5, 0.8])
+    spec = dict(k=(2, -1, 3), e=tuple(e / np.linalg.norm(e)), phi=0.7, f0=0.05, dt=0.02)  # e need not be normal to k
+    f = O.rhs(np.zeros((4, n, n, n)), dx, 0.01, cs, P55, force=spec)  # uniform state at rest: the RHS is f alone (P5)
+    N, fk = _forcing_expected(spec, cs)
+    assert abs(N - 0.05 * 1.3 * math.sqrt(math.sqrt(14.0) * 1.3 / 0.02)) < 1e-15  # Eq. 25 with the numbers put in
+    assert abs(np.dot(fk, spec["k"])) < 1e-15 and abs(np.dot(fk, spec["e"])) < 1e-15  # solenoidal, normal to e
+    assert np.array_equal(f[0], np.zeros((n, n, n)))  # no source in the continuity equation
+    for a in range(3):
+        spec_a = np.fft.fftn(f[1 + a]) / n ** 3  # array axes are (z, y, x)
+        peak = spec_a[3, -1, 2]  # the +k mode
+        assert abs(peak - 0.5 * N * fk[a] * np.exp(1j * 0.7)) < 1e-14
+        spec_a[3, -1, 2] = spec_a[-3, 1, -2] = 0
+        assert np.abs(spec_a).max() < 1e-15  # and nothing else
+    # the 19-point path carries the same f
+    assert np.array_equal(O.rhs(np.zeros((4, n, n, n)), dx, 0.01, cs, P19, force=spec), f)
+
+
+@pytest.mark.parametrize("path", [P55, P19])
+def test_p13_forcing_adds_to_the_rhs_and_leaves_it_when_switched_off(path):
+    cfg = I.CONFIGS["C1"]
+    F = I.make_state(cfg, n_override=12)
+    dx = TWO_PI / 12
+    spec = dict(k=(1, 2, 0), e=(0, 0, 1), phi=-1.1, f0=0.3, dt=0.01)
+    plain = O.rhs(F, dx, cfg.nu, cfg.cs, path)
+    forced = O.rhs(F, dx, cfg.nu, cfg.cs, path, force=spec)
+    f = O.rhs(np.zeros_like(F), dx, cfg.nu, cfg.cs, path, force=spec)
+    assert relinf(forced - plain, f) < 1e-13
+    assert np.array_equal(O.rhs(F, dx, cfg.nu, cfg.cs, path), plain)  # the context manager switched it off again
+    with pytest.raises(ValueError):
+        O.rhs(F, dx, cfg.nu, cfg.cs, path, force=dict(k=(0, 0, 2), e=(0, 0, 1), phi=0, f0=1, dt=0.01))  # k parallel to e
+
+
+@pytest.mark.parametrize("path", [P55, P19])
+@pytest.mark.parametrize("axis,e", [(0, (0, 0, 1)), (1, (1, 0, 0)), (2, (0, 1, 0))])
+def test_p13_forced_shear_mode_from_rest_closed_form(path, axis, e):
+    """k along an axis: f is a transverse shear mode, every nonlinear term and div u vanish identically in the discrete
+    system, and u = a_n f_k cos(k x + phi) with the inhomogeneous RK3 recurrence a_{n+1} = G a_n + N dt (G - 1)/z,
+    G = 1 + z + z^2/2 + z^3/6, z = -nu dt s2(k dx)/dx^2 — which pins that f enters w with the weight dt of Eq. 10, on
+    all three substeps, with N formed from the step's own dt."""
+    n, kk, nu, nsteps = 24, 3, 0.02, 7
+    dx = TWO_PI / n
+    dt = 0.1 * dx
+    kvec = [0, 0, 0]
+    kvec[axis] = kk
+    spec = dict(k=tuple(kvec), e=e, phi=0.4, f0=0.02, dt=dt)
+    out = O.rk3_step(np.zeros((4, n, n, n)), dx, nu, 1.0, dt, nsteps, path, force=spec)
+    N, fk = _forcing_expected(spec, 1.0)
+    z = -nu * dt * s2(kk * dx) / dx ** 2
+    G = 1 + z + z * z / 2 + z ** 3 / 6
+    a = 0.0
+    for _ in range(nsteps):
+        a = G * a + N * dt * (1 + z / 2 + z * z / 6)
+    idx = np.arange(n) * dx
+    shape = [1, 1, 1]
+    shape[2 - axis] = n
+    c = np.cos(kk * idx + 0.4).reshape(shape)
+    assert np.abs(out[0]).max() < 1e-16
+    for comp in range(3):
+        np.testing.assert_allclose(out[1 + comp], a * fk[comp] * c * np.ones((n, n, n)), atol=2e-15 * abs(a))
+    assert abs(a) > 1e-3  # the test is not vacuous
+
+
+def test_p13_windowed_forced_step_equals_the_full_grid_step():
+    rng = np.random.default_rng(3)
+    n = 40
+    F = 0.05 * rng.standard_normal((4, n, n, n))
+    dx = TWO_PI / n
+    spec = dict(k=(2, 1, -1), e=(0, 0, 1), phi=0.2, f0=0.1, dt=0.1 * dx)
+    full = O.rk3_step(F, dx, 5e-3, 1.0, 0.1 * dx, 1, P55, force=spec)
+    m = O.window_margin(P55)
+    origin = (n - m - 2, 5 - m, 20 - m)  # (k0, j0, i0) of the block's first cell; the oracle takes (x, y, z) order
+    sub = I.gather_block(F, origin, 4 + 2 * m)
+    got = O.rk3_step(sub, dx, 5e-3, 1.0, 0.1 * dx, 1, P55, force=spec, origin=origin[::-1])[:, m:-m, m:-m, m:-m]
+    exp = I.gather_block(full, tuple(o + m for o in origin), 4)
+    assert relinf(got, exp) < 1e-13  # the phase k.x of a shifted origin differs from the full grid's by rounding only
