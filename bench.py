@@ -199,6 +199,8 @@ def main():
     ap.add_argument("--path", default="55", choices=["55", "19"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 direct, 2 tiled, 3 paired")
+    ap.add_argument("--forcing", action="store_true",
+                    help="switch the forcing term of Eq. 2 on (Eq. 24-25; off in the paper's performance runs, PAPER.md:369)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=15.0)
     args = ap.parse_args()
@@ -237,6 +239,9 @@ def main():
     if args.variant:
         ctx.fd_set_variant(args.variant)
     info = ctx.fd_get_info()
+    forcing = dict(k=(3.0, 2.0, -4.0), e=(0.36, -0.48, 0.8), phi=0.7, f0=0.05) if args.forcing else None
+    if forcing:
+        ctx.fd_set_forcing(forcing["k"], forcing["e"], forcing["phi"], forcing["f0"], cfg.dt)
     ctx.load_state(F0)
     ctx.fd_rk3_step(cfg.dt, W)  # warm-up
     ctx.load_state(F0)          # timed steps start from the config's state
@@ -319,7 +324,8 @@ def main():
                                    f"nu={cfg.nu}, dt=0.1 dx/cs", "path": f"{args.path}-point",
                        "variant": {1: "direct", 2: "tiled", 3: "paired"}.get(info.variant, str(info.variant)),
                        "l2": "inputs larger than L2 (2.1 GB state, 8.6 GB streamed per substep); no flush needed",
-                       "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite},
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite,
+                       "forcing": (f"on: k={forcing['k']}, f0={forcing['f0']}" if forcing else "off (PAPER.md:369)")},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
                     "d2h_bytes_per_step": state_bytes / K,
                     "job": f"fd_load(host pinned) + fd_rk3_step(dt,{K}) + fd_store(host pinned)", "ms": e2e_ms,

@@ -85,6 +85,16 @@ int fd_set_path(fd_ctx* ctx, int path);
 int fd_set_variant(fd_ctx* ctx, int variant);
 int fd_set_stream(fd_ctx* ctx, void* cuda_stream);
 
+/* Forcing term f of Eq. 2 (Eq. 24-25), frozen until the next call:
+ *     f(x) = Re{ N f_k exp(i k.x + i phi) } = N f_k cos(k.x + phi),   x = (i, j, k) * dx (cell (0,0,0) at the origin),
+ *     N = f0 cs sqrt(|k| cs / dt_ref),   f_k = (k x e) / sqrt(|k|^2 - (k.e)^2).
+ * k, e: 3 doubles each (host); k should be 2 pi / (n dx) times integers for f to be periodic on the grid; dt_ref is the
+ * step size N is formed with (normally the dt later given to fd_rk3_step).  f is added to the momentum right-hand side
+ * on all three substeps of every following fd_rk3_step and to fd_rhs, on both stencil paths.  f0 = 0 switches the
+ * forcing off (the default, and the setting of the paper's performance runs); k and e may then be NULL.
+ * FD_EINVAL: f0 < 0 or not finite, NULL or non-finite k/e/phi, dt_ref <= 0, k parallel to e.  Synchronises the stream. */
+int fd_set_forcing(fd_ctx* ctx, const double* k, const double* e, double phi, double f0, double dt_ref);
+
 /* Copy the caller's four fields in (and fill the ghost zones) / copy the current fields out. */
 int fd_load(fd_ctx* ctx, const void* lnrho, const void* ux, const void* uy, const void* uz, int where);
 int fd_store(fd_ctx* ctx, void* lnrho, void* ux, void* uy, void* uz, int where);

@@ -83,6 +83,10 @@ struct fd_ctx {
     double prof_ms[FD_K_COUNT] = {};
     unsigned long long prof_n[FD_K_COUNT] = {};
     TiledState tiled;  // tensor maps etc. of the tiled variant
+    // forcing term of Eq. 2 (fd_set_forcing): amplitude N f_k and the device table of the separable phase
+    bool force_on = false;
+    double famp[3] = {0, 0, 0};
+    void* ftab = nullptr;
 };
 
 static int ctx_alloc(fd_ctx* c, void** p, size_t bytes) {
@@ -178,6 +182,7 @@ static Coef<T> make_coef(const fd_ctx* c) {
     k.nu = T(S(c->nu));
     k.nu3 = T(S(c->nu / 3.0));
     k.cs2 = T(S(c->cs * c->cs));
+    for (int a = 0; a < 3; ++a) k.fa[a] = T(S(c->force_on ? c->famp[a] : 0.0));
     return k;
 }
 
@@ -266,17 +271,25 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
     T* Div = (T*)c->Div;
     const bool p55 = c->path == FD_PATH_55;
     const bool tiled = c->variant == FD_VARIANT_TILED || c->variant == FD_VARIANT_PAIRED;
+    ForceTab<T> ft;
+    ft.tab = c->force_on ? (const typename Scalar<T>::type*)c->ftab : nullptr;
+    ft.nx = c->nx;
+    ft.ny = c->ny;
+    ft.nzc = c->nz;
+    const double no_force[3] = {0, 0, 0};
     dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
     {
         LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
         if (tiled) {
-            const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w);
-            if (tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, c->stream))
-                return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w,
+                                        c->force_on ? c->famp : no_force);
+            const int lrc = tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, ft, c->stream);
+            if (lrc == 4) return fail(FD_EUNSUPPORTED, "forcing on a grid with this many planes needs FD_VARIANT_DIRECT");
+            if (lrc) return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         } else if (p55) {
-            k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s);
+            k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s, ft);
         } else {
-            k_direct_main<T, false><<<grid, block, 0, c->stream>>>(Fin, Fout, W, Div, g, k, s);
+            k_direct_main<T, false><<<grid, block, 0, c->stream>>>(Fin, Fout, W, Div, g, k, s, ft);
         }
     }
     if (!p55) {
@@ -554,6 +567,7 @@ extern "C" int fd_destroy(fd_ctx* c) {
     ctx_free(c, c->F[1]);
     ctx_free(c, c->W);
     ctx_free(c, c->Div);
+    ctx_free(c, c->ftab);
     cudaGetLastError();
     delete c;
     return FD_OK;
@@ -579,6 +593,53 @@ extern "C" int fd_set_variant(fd_ctx* c, int variant) {
     int rc = resolve_variant(c);
     if (rc) c->variant_req = old;
     return rc;
+}
+
+extern "C" int fd_set_forcing(fd_ctx* c, const double* k, const double* e, double phi, double f0, double dt_ref) {
+    FD_CHECK_CTX(c);
+    if (!std::isfinite(f0) || f0 < 0) return fail(FD_EINVAL, "fd_set_forcing: f0 must be finite and >= 0");
+    if (f0 == 0) {
+        c->force_on = false;
+        return FD_OK;
+    }
+    if (!k || !e) return fail(FD_EINVAL, "fd_set_forcing: NULL vector");
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(k[a]) || !std::isfinite(e[a])) return fail(FD_EINVAL, "fd_set_forcing: non-finite vector");
+    if (!std::isfinite(phi) || !(dt_ref > 0) || !std::isfinite(dt_ref)) return fail(FD_EINVAL, "fd_set_forcing: bad phi or dt_ref");
+    const double k2 = k[0] * k[0] + k[1] * k[1] + k[2] * k[2], ke = k[0] * e[0] + k[1] * e[1] + k[2] * e[2];
+    const double den2 = k2 - ke * ke;
+    if (!(den2 > 0)) return fail(FD_EINVAL, "fd_set_forcing: k must not be parallel to e (|k|^2 - (k.e)^2 > 0)");
+    // Eq. 25:  N = f0 cs sqrt(|k| cs / dt),  f_k = (k x e) / sqrt(|k|^2 - (k.e)^2)
+    const double N = f0 * c->cs * std::sqrt(std::sqrt(k2) * c->cs / dt_ref), den = std::sqrt(den2);
+    c->famp[0] = N * (k[1] * e[2] - k[2] * e[1]) / den;
+    c->famp[1] = N * (k[2] * e[0] - k[0] * e[2]) / den;
+    c->famp[2] = N * (k[0] * e[1] - k[1] * e[0]) / den;
+    // separable phase tables, formed in double and rounded once: cx sx (with phi) | cy sy | cz sz
+    const int n[3] = {c->nx, c->ny, c->nz};
+    const size_t count = 2 * ((size_t)n[0] + n[1] + n[2]), ssize = c->dtype == FD_F64 ? 8 : 4;
+    if (!c->ftab) {
+        int rc = ctx_alloc(c, &c->ftab, count * ssize);
+        if (rc) return rc;
+    }
+    std::vector<double> tab(count);
+    size_t off = 0;
+    for (int a = 0; a < 3; ++a) {
+        for (int i = 0; i < n[a]; ++i) {
+            const double th = k[a] * (i * c->dx) + (a == 0 ? phi : 0.0);
+            tab[off + i] = std::cos(th);
+            tab[off + n[a] + i] = std::sin(th);
+        }
+        off += 2 * (size_t)n[a];
+    }
+    if (c->dtype == FD_F64) {
+        FD_CUDA(cudaMemcpyAsync(c->ftab, tab.data(), count * 8, cudaMemcpyHostToDevice, c->stream));
+    } else {
+        std::vector<float> tf(tab.begin(), tab.end());
+        FD_CUDA(cudaMemcpyAsync(c->ftab, tf.data(), count * 4, cudaMemcpyHostToDevice, c->stream));
+    }
+    FD_CUDA(cudaStreamSynchronize(c->stream));  // the host tables go out of scope
+    c->force_on = true;
+    return FD_OK;
 }
 
 extern "C" int fd_set_stream(fd_ctx* c, void* s) {

@@ -52,6 +52,33 @@ __device__ __forceinline__ V2 zwrap<V2>(V2 v) { return V2(v.v.y, v.v.x); }
 template <class T> struct Scalar { typedef T type; static constexpr int lanes = 1; };
 template <> struct Scalar<V2> { typedef float type; static constexpr int lanes = 2; };
 
+// make_value<T>(lo, hi): a value from the scalars of its cell(s): lo for a plain type, (lo, hi) for a V2 pair.
+template <class T> __host__ __device__ __forceinline__ T make_value(typename Scalar<T>::type lo, typename Scalar<T>::type) { return T(lo); }
+template <> __host__ __device__ __forceinline__ V2 make_value<V2>(float lo, float hi) { return V2(lo, hi); }
+
+// Forcing term of Eq. 2 (Eq. 24-25):  f = N f_k cos(k.x + phi), x = (i, j, k) dx.  The phase is
+// separable, so the host tabulates (in double, rounded once) cos and sin of k_x x_i + phi, of k_y y_j and of k_z z_k;
+// `tab` holds them back to back as scalars: cx[nx] sx[nx] cy[ny] sy[ny] cz[nzc] sz[nzc], nzc = the CALLER's nz.
+// A kernel forms cos(theta) = cxy cz - sxy sz with cxy = cx cy - sx sy, sxy = sx cy + cx sy.
+template <class T>
+struct ForceTab {
+    const typename Scalar<T>::type* tab;  // NULL: forcing off
+    int nx, ny, nzc;
+    __device__ __forceinline__ void xy(int i, int j, T& cxy, T& sxy) const {
+        typedef typename Scalar<T>::type S;
+        const S cx = tab[i], sx = tab[nx + i], cy = tab[2 * nx + j], sy = tab[2 * nx + ny + j];
+        cxy = T(cx * cy - sx * sy);
+        sxy = T(sx * cy + cx * sy);
+    }
+    // stored plane z holds cells z (and z + nzc/2 in the paired layout)
+    __device__ __forceinline__ void z(int zz, T& cz, T& sz) const {
+        const typename Scalar<T>::type* c = tab + 2 * nx + 2 * ny;
+        const int hi = Scalar<T>::lanes == 2 ? zz + nzc / 2 : zz;
+        cz = make_value<T>(c[zz], c[hi]);
+        sz = make_value<T>(c[nzc + zz], c[nzc + hi]);
+    }
+};
+
 // Ghost-padded array geometry, in units of the value type T of the kernels (one cell,
 // or a V2 pair of cells: then nz is HALF the caller's nz).  Value (i,j,k) of a padded field lives at
 //   (i + gx) + px * ((j + gy) + py * (k + gz));  the four fields of one copy are fs values apart.
@@ -70,6 +97,7 @@ struct Coef {
     T b0, b1, b2, b3;  // Eq. 7: -490, 270, -27, 2 over 180 dx^2
     T m1, m2, m3;      // Eq. 8:  270, -27, 2 over 720 dx^2
     T nu, nu3, cs2;    // nu, nu/3, cs^2
+    T fa[3];           // N f_k of the forcing term (Eq. 24-25); used only when a ForceTab is given
 };
 
 // One RK substep (Eq. 10):  w <- alpha w + dt rhs ; F_out <- F + beta w.

@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfi
 // ------------------------------------------------------------------------------------------------
 template <class T, bool PATH55>
 __global__ void __launch_bounds__(256) k_direct_main(const T* __restrict__ Fin, T* __restrict__ Fout, T* __restrict__ W,
-                                                     T* __restrict__ Div, Geom g, Coef<T> c, Sub<T> s) {
+                                                     T* __restrict__ Div, Geom g, Coef<T> c, Sub<T> s, ForceTab<T> ft) {
     int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
     if (i >= g.nx || j >= g.ny) return;
     const long long sx = 1, sy = g.px, sz = (long long)g.px * g.py;
@@ -172,6 +172,14 @@ __global__ void __launch_bounds__(256) k_direct_main(const T* __restrict__ Fin, 
     }
     T Rv[4];
     assemble<T, PATH55>(u, gl, G, L, Q, c, Rv);
+    if (ft.tab) {  // + f = N f_k cos(k.x + phi) (Eq. 2, Eq. 24-25)
+        T cxy, sxy, cz, sz;
+        ft.xy(i, j, cxy, sxy);
+        ft.z(k, cz, sz);
+        const T cth = cxy * cz - sxy * sz;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) Rv[1 + a] += c.fa[a] * cth;
+    }
     if (!PATH55) Div[p] = G[0][0] + G[1][1] + G[2][2];
     const T fc[4] = {l[0], u[0], u[1], u[2]};
 #pragma unroll

@@ -46,6 +46,7 @@ struct KC {
     T mq[3];   // dt (nu / 3) c_m / (720 dx^2)              Eq. 8
     T nu, nu2, nu23, cs2dt, dt;
     T alpha, beta;
+    T fa[3];   // FORCE: dt N f_k (Eq. 24-25), the amplitude of the forcing term in dt*rhs_i
     int read_w, write_f, write_w;
 };
 
@@ -191,7 +192,8 @@ struct Regs6 {
 };
 
 // TX x TY threads; a thread owns RY vertically adjacent columns (rows cj .. cj+RY-1), so the tile is TX x (TY*RY).
-template <class T, bool PATH55, int TX, int TY, int NS_, int RY>
+// FORCE: the forcing term of Eq. 2 is added (a separate instantiation, so the unforced kernel pays nothing).
+template <class T, bool PATH55, int TX, int TY, int NS_, int RY, bool FORCE>
 struct Tiled {
     static constexpr int TH = TY * RY;  // tile height in values
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
@@ -211,10 +213,12 @@ struct Tiled {
     // columns (6 values) + 4 fields x 8 window slots of 2 columns = 128 columns.  TMEM is otherwise idle here.
     static constexpr bool TM = sizeof(T) == 8;
     static constexpr int DLCOLS = 16, TWIN = 4 * DLCOLS, TBLOCK = TWIN + 4 * 16;
+    static constexpr int FXYCOL = 12;  // spare columns 12..15 of delay-line slot 0: the forcing's xy phase factors
     static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * RY * TBLOCK;
     static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
     static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
-    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 1) * sizeof(uint64_t);
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 2) * sizeof(uint64_t);
+    static size_t smem_bytes(int planes) { return SMEM + (FORCE ? 2 * (size_t)planes * sizeof(T) : 0); }  // + the z table
     static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
     struct State {   // of one owned column
@@ -236,11 +240,13 @@ struct Tiled {
 
     // One plane.  sp0: the thread's first centre in stage 0 of the F ring; wsp0: its first element in stage 0 of the
     // w ring; gF, gW, gD: its first cell of output plane z = t - 3 in F_out, w and div (field strides fs, n; row
-    // pitches pf, pw); `out`: that plane is produced; ok[r]: owned column r lies inside the grid.
+    // pitches pf, pw); `out`: that plane is produced; ok[r]: owned column r lies inside the grid.  FORCE: ftz points
+    // at (cos, sin) of k_z z of the output plane in shared memory; cos and sin of k_x x + k_y y + phi of the owned
+    // columns sit in four spare tensor-memory columns (8-byte types) or are re-read from the tables ft (plain fp32).
     template <int PH>
     static __device__ __forceinline__ void step(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
                                                 const KC<T>& c, bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
-                                                long long n, int pf, int pw, const bool (&ok)[RY]) {
+                                                long long n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
         const T* sp = sp0 + (PH & (NS - 1)) * STAGE;
         // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8).  The RY + 6 values of the thread's own
@@ -353,6 +359,7 @@ struct Tiled {
         // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
         constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
         const T* wsp = wsp0 + ((PH + 2) & 3) * WSTAGE;  // w ring slot of plane index p - 6
+        uint32_t fr[RY][4];  // FORCE && TM: cos, sin of the xy phase of the owned columns, from tensor memory
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
             T d1z[4], fc[4], del[6];
@@ -364,6 +371,7 @@ struct Tiled {
                 for (int f = 0; f < 4; ++f) tmem_ld16(tdl + r * TBLOCK + TWIN + f * 16, wr[f]);
                 tmem_ld<8>(tdl + r * TBLOCK + r4 * DLCOLS, dr);
                 tmem_ld<4>(tdl + r * TBLOCK + r4 * DLCOLS + 8, dr + 8);
+                if constexpr (FORCE) tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr[r]);
                 tmem_wait_ld();
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
@@ -418,6 +426,19 @@ struct Tiled {
             Rv[1] = rx;
             Rv[2] = ry;
             Rv[3] = rz;
+            if constexpr (FORCE) {  // + dt f_i = dt N f_k,i cos(k.x + phi), cos(a + b) = cos a cos b - sin a sin b
+                T cxy = T(0), sxy = T(0);
+                if constexpr (TM) {
+                    const uint2 uc = make_uint2(fr[r][0], fr[r][1]), us = make_uint2(fr[r][2], fr[r][3]);
+                    cxy = *reinterpret_cast<const T*>(&uc);
+                    sxy = *reinterpret_cast<const T*>(&us);
+                } else if (ok[r]) {
+                    ft.xy(ci, cj + r, cxy, sxy);  // L1-resident tables: no registers held across planes
+                }
+                const T cth = fma_(-sxy, ftz[1], cxy * ftz[0]);
+#pragma unroll
+                for (int i = 0; i < 3; ++i) Rv[1 + i] = fma_(c.fa[i], cth, Rv[1 + i]);
+            }
             // ---- Eq. 10; coalesced row segments per warp straight to global memory
             if (ok[r]) {
 #pragma unroll
@@ -432,7 +453,7 @@ struct Tiled {
     }
 
     static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, const Sched sc, T* __restrict__ Fout,
-                                               T* __restrict__ W, T* __restrict__ Div) {
+                                               T* __restrict__ W, T* __restrict__ Div, const ForceTab<T>& ft) {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
         T* smw = sm + NS * STAGE;
@@ -468,6 +489,11 @@ struct Tiled {
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
         const uint32_t a_tmem = a_wfull + 8 * NW;  // shared word that receives the TMEM base address
+        // FORCE: (cos, sin) of k_z z for the output planes of this item, behind the barriers
+        T* ftz = reinterpret_cast<T*>(smem_raw + (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 2) * sizeof(uint64_t));
+        if constexpr (FORCE) {
+            for (int i = tid; i < ze - zs; i += THREADS) ft.z(zs + i, ftz[2 * i], ftz[2 * i + 1]);
+        }
         uint32_t tmem_base = 0;
         if constexpr (TM) {
             if (tid < 32) {  // warp 0 allocates (and frees) the tensor-memory columns
@@ -497,6 +523,16 @@ struct Tiled {
 #pragma unroll
         for (int r = 0; r < RY; ++r) ok[r] = ci < g.nx && cj + r < g.ny;
         const bool store_ok = ok[0];
+        if constexpr (FORCE && TM) {
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                T cxy = T(0), sxy = T(0);
+                if (ok[r]) ft.xy(ci, cj + r, cxy, sxy);
+                const uint2 uc = *reinterpret_cast<const uint2*>(&cxy), us = *reinterpret_cast<const uint2*>(&sxy);
+                const uint32_t r4[4] = {uc.x, uc.y, us.x, us.y};
+                tmem_st<4>(tdl + r * TBLOCK + FXYCOL, r4);
+            }
+        }
         const long long plane_w = (long long)g.nx * g.ny, plane_f = (long long)g.px * g.py;
         long long ow = ci + (long long)g.nx * (cj + (long long)g.ny * zs);
         long long of = (ci + g.gx) + (long long)g.px * ((cj + g.gy) + (long long)g.py * (zs + g.gz));
@@ -526,7 +562,8 @@ struct Tiled {
                     if constexpr (TM) tmem_wait_st();  // what the previous planes parked in tensor memory is in place
                     mbar_wait(a_full + 8 * (ph & (NS - 1)), (uint32_t)((p >> LNS) & 1));
                     if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
-#define FD6_STEP(K) step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, g.px, g.nx, ok)
+#define FD6_STEP(K) \
+    step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R))
                     switch (ph) {  // ph is a compile-time constant after unrolling
                         case 0: FD6_STEP(0); break;
                         case 1: FD6_STEP(1); break;
@@ -574,11 +611,11 @@ struct Tiled {
     }
 };
 
-template <class T, bool PATH55, int TX, int TY, int NS, int RY>
+template <class T, bool PATH55, int TX, int TY, int NS, int RY, bool FORCE>
 __global__ void __launch_bounds__(TX* TY, 1)
     k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, const Sched sc, T* __restrict__ Fout,
-                 T* __restrict__ W, T* __restrict__ Div) {
-    Tiled<T, PATH55, TX, TY, NS, RY>::run(m, g, c, sc, Fout, W, Div);
+                 T* __restrict__ W, T* __restrict__ Div, const ForceTab<T> ft) {
+    Tiled<T, PATH55, TX, TY, NS, RY, FORCE>::run(m, g, c, sc, Fout, W, Div, ft);
 }
 
 // Tile shape per value type (registers per thread bound the CTA size).  RY = 2 (two vertically
@@ -607,6 +644,7 @@ typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_
 struct TiledState {
     bool ready = false;
     Maps maps[2];      // maps[cur]: read copy F[cur]
+    bool force_fits = true;  // the forcing's z table fits in shared memory beside the rings
     Sched sched{};     // work list
     int items = 0;     // grid size
     int sm_count = 0;
@@ -695,11 +733,15 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
         if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY * RY, 4);
     }
     if (rc) return rc;
-    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)Tiled<T, true, TX, TY, NS, RY>::SMEM);
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 (int)Tiled<T, false, TX, TY, NS, RY>::SMEM);
+    const int smem = (int)Tiled<T, true, TX, TY, NS, RY, false>::SMEM;  // the same for all four instantiations
+    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    const int smem_f = (int)Tiled<T, true, TX, TY, NS, RY, true>::smem_bytes(g.nz);  // + the forcing's z table
+    ts.force_fits = smem_f <= 227 * 1024;
+    if (ts.force_fits) {
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_f);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_f);
+    }
     if (e != cudaSuccess) {
         snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
         cudaGetLastError();
@@ -719,7 +761,7 @@ inline void tiled_release(TiledState& ts) { ts.ready = false; }
 
 template <class T>
 static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, double alpha, double beta, int read_w, int write_f,
-                     int write_w) {
+                     int write_w, const double famp[3]) {
     typedef typename Scalar<T>::type S;
     const double dx2 = dx * dx;
     const double b[4] = {-490.0 / (180.0 * dx2), 270.0 / (180.0 * dx2), -27.0 / (180.0 * dx2), 2.0 / (180.0 * dx2)};
@@ -746,6 +788,7 @@ static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
     k.dt = T(S(dt));
     k.alpha = T(S(alpha));
     k.beta = T(S(beta));
+    for (int i = 0; i < 3; ++i) k.fa[i] = T(S(dt * famp[i]));
     k.read_w = read_w;
     k.write_f = write_f;
     k.write_w = write_w;
@@ -756,13 +799,23 @@ static KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
 // leaves dt * div u in Div): reads copy `cur`, writes copy 1 - cur and w.
 template <class T>
 static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
-                             cudaStream_t stream) {
+                             const ForceTab<T>& ft, cudaStream_t stream) {
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
+    constexpr size_t SMEM = Tiled<T, true, TX, TY, NS, RY, false>::SMEM;
     dim3 block(TX, TY, 1), grid(ts.items, 1, 1);
-    if (path55)
-        k_tiled_main<T, true, TX, TY, NS, RY><<<grid, block, Tiled<T, true, TX, TY, NS, RY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
-    else
-        k_tiled_main<T, false, TX, TY, NS, RY><<<grid, block, Tiled<T, false, TX, TY, NS, RY>::SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div);
+    if (ft.tab == nullptr) {
+        if (path55)
+            k_tiled_main<T, true, TX, TY, NS, RY, false><<<grid, block, SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+        else
+            k_tiled_main<T, false, TX, TY, NS, RY, false><<<grid, block, SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+    } else {
+        if (!ts.force_fits) return 4;
+        const size_t smem_f = Tiled<T, true, TX, TY, NS, RY, true>::smem_bytes(g.nz);
+        if (path55)
+            k_tiled_main<T, true, TX, TY, NS, RY, true><<<grid, block, smem_f, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+        else
+            k_tiled_main<T, false, TX, TY, NS, RY, true><<<grid, block, smem_f, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+    }
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 

@@ -25,7 +25,7 @@ EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
     "fd_rhs", "fd_rk3_step", "fd_sync", "fd_destroy", "fd_last_error", "fd_get_info", "fd_kernel_launches",
     "fd_set_profiling", "fd_get_profile", "fd_reset_profile", "fd_debug_poison_w", "fd_debug_poison_ghosts",
-    "fd_plan_work_list",
+    "fd_plan_work_list", "fd_set_forcing",
 ]
 
 if not os.path.exists(_LIB_PATH):
@@ -72,6 +72,7 @@ lib.fd_get_profile.argtypes = [_vp, _i, C.POINTER(_d), C.POINTER(C.c_ulonglong)]
 lib.fd_reset_profile.argtypes = [_vp]
 lib.fd_debug_poison_w.argtypes = [_vp]
 lib.fd_debug_poison_ghosts.argtypes = [_vp]
+lib.fd_set_forcing.argtypes = [_vp, C.POINTER(_d), C.POINTER(_d), _d, _d, _d]
 lib.fd_plan_work_list.argtypes = [_i, _i, _i, _i, _i, C.POINTER(FdWorkList)]
 
 
@@ -160,6 +161,13 @@ class Fd:
 
     def fd_set_variant(self, variant):
         _check(lib.fd_set_variant(self._h, variant))
+
+    def fd_set_forcing(self, k, e, phi, f0, dt_ref):
+        """Forcing term of Eq. 2 (Eq. 24-25); f0 = 0 switches it off (k, e may then be None)."""
+        self._stream()
+        kv = (C.c_double * 3)(*[float(v) for v in k]) if k is not None else None
+        ev = (C.c_double * 3)(*[float(v) for v in e]) if e is not None else None
+        _check(lib.fd_set_forcing(self._h, kv, ev, float(phi), float(f0), float(dt_ref)))
 
     def fd_load(self, lnrho, ux, uy, uz, where):
         self._stream()

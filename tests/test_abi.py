@@ -70,6 +70,7 @@ def test_argument_validation_happens_before_any_cuda_call(fd6):
     assert L.fd_set_path(None, 0) == fd6.FD_EINVAL
     assert L.fd_destroy(None) == fd6.FD_OK
     assert L.fd_kernel_launches(None) == 0
+    assert L.fd_set_forcing(None, None, None, 0.0, 0.0, 1.0) == fd6.FD_EINVAL
 
 
 def test_no_cpu_fallback_without_a_device(fd6):
