@@ -214,6 +214,9 @@ struct Tiled {
     static constexpr bool TM = sizeof(T) == 8;
     static constexpr int DLCOLS = 16, TWIN = 4 * DLCOLS, TBLOCK = TWIN + 4 * 16;
     static constexpr int FXYCOL = 12;  // spare columns 12..15 of delay-line slot 0: the forcing's xy phase factors
+    // when to fetch them: with the window (fp64) or after the right-hand side is assembled (paired fp32, where the
+    // register pressure peaks at the window load: 144 registers and no spill instead of 168 with spills) — measured
+    static constexpr bool FXY_LATE = Scalar<T>::lanes == 2;
     static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * RY * TBLOCK;
     static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
     static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
@@ -359,10 +362,10 @@ struct Tiled {
         // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
         constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
         const T* wsp = wsp0 + ((PH + 2) & 3) * WSTAGE;  // w ring slot of plane index p - 6
-        uint32_t fr[RY][4];  // FORCE && TM: cos, sin of the xy phase of the owned columns, from tensor memory
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
             T d1z[4], fc[4], del[6];
+            uint32_t fr[4];  // FORCE && TM: cos, sin of the xy phase of the owned column, from tensor memory
             if constexpr (TM) {
                 // the whole window ring of a field is 16 consecutive columns: one load each; slot t of this plane may
                 // still be in flight, so it is taken from the register that holds it
@@ -371,7 +374,7 @@ struct Tiled {
                 for (int f = 0; f < 4; ++f) tmem_ld16(tdl + r * TBLOCK + TWIN + f * 16, wr[f]);
                 tmem_ld<8>(tdl + r * TBLOCK + r4 * DLCOLS, dr);
                 tmem_ld<4>(tdl + r * TBLOCK + r4 * DLCOLS + 8, dr + 8);
-                if constexpr (FORCE) tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr[r]);
+                if constexpr (FORCE && !FXY_LATE) tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr);
                 tmem_wait_ld();
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
@@ -429,7 +432,11 @@ struct Tiled {
             if constexpr (FORCE) {  // + dt f_i = dt N f_k,i cos(k.x + phi), cos(a + b) = cos a cos b - sin a sin b
                 T cxy = T(0), sxy = T(0);
                 if constexpr (TM) {
-                    const uint2 uc = make_uint2(fr[r][0], fr[r][1]), us = make_uint2(fr[r][2], fr[r][3]);
+                    if constexpr (FXY_LATE) {
+                        tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr);
+                        tmem_wait_ld();
+                    }
+                    const uint2 uc = make_uint2(fr[0], fr[1]), us = make_uint2(fr[2], fr[3]);
                     cxy = *reinterpret_cast<const T*>(&uc);
                     sxy = *reinterpret_cast<const T*>(&us);
                 } else if (ok[r]) {
