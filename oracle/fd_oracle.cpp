@@ -14,7 +14,7 @@
 //     reference legs may load the library built from it.
 //
 // Parity status: every function below is pinned by tests/test_oracle_pins.py
-// (P1..P10 of DESIGN.md) EXCEPT the nonlinear multi-step evolution of general
+// (P0..P13 of DESIGN.md; the forcing term O11 by P13) EXCEPT the nonlinear multi-step evolution of general
 // fields beyond one substep, which is "parity unpinned beyond the oracle itself"
 // (it is pinned only through the per-substep closed form P3, the linear closed
 // form P6 and the 19-vs-55 O(dx^6) agreement).
