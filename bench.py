@@ -54,7 +54,7 @@ class ClockSampler:
 
     def __init__(self, index, period=0.01):
         self.index, self.period = index, period
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.power, self.reasons, self.max_mhz = [], [], set(), None
         self._stop = threading.Event()
         self._thr = None
         try:
@@ -79,6 +79,10 @@ class ClockSampler:
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
                 try:
+                    self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                except Exception:
+                    pass
+                try:
                     mask = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
                 except Exception:
                     mask = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
@@ -102,7 +106,8 @@ class ClockSampler:
 
     def summary(self):
         s = sorted(self.samples)
-        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_mhz_min": (s[0] if s else None), "sm_max_mhz": self.max_mhz,
+                "power_w_max": (round(max(self.power), 1) if self.power else None),
                 "reasons": sorted(self.reasons), "samples": len(s)}
 
 
