@@ -242,14 +242,14 @@ struct Tiled {
     }
 
     // One plane.  sp0: the thread's first centre in stage 0 of the F ring; wsp0: its first element in stage 0 of the
-    // w ring; gF, gW, gD: its first cell of output plane z = t - 3 in F_out, w and div (field strides fs, n; row
+    // w ring; bF, bW, bD + of / ow: its first cell of output plane z = t - 3 in F_out, w and div (field strides fs, n; row
     // pitches pf, pw); `out`: that plane is produced; ok[r]: owned column r lies inside the grid.  FORCE: ftz points
     // at (cos, sin) of k_z z of the output plane in shared memory; cos and sin of k_x x + k_y y + phi of the owned
     // columns sit in four spare tensor-memory columns (8-byte types) or are re-read from the tables ft (plain fp32).
     template <int PH>
     static __device__ __forceinline__ void step(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
-                                                const KC<T>& c, bool out, T* __restrict__ gF, T* __restrict__ gW, T* __restrict__ gD, long long fs,
-                                                long long n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
+                                                const KC<T>& c, bool out, T* __restrict__ bF, T* __restrict__ bW, T* __restrict__ bD, uint32_t of, uint32_t ow,
+                                                uint32_t fs, uint32_t n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
         const T* sp = sp0 + (PH & (NS - 1)) * STAGE;
         // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8).  The RY + 6 values of the thread's own
@@ -451,10 +451,10 @@ struct Tiled {
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
                     const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD + r * TX], Rv[f]) : Rv[f];
-                    if (c.write_w) gW[f * n + r * pw] = wn;
-                    if (c.write_f) gF[f * fs + r * pf] = fma_(c.beta, wn, fc[f]);
+                    if (c.write_w) bW[ow + f * n + r * pw] = wn;
+                    if (c.write_f) bF[of + f * fs + r * pf] = fma_(c.beta, wn, fc[f]);
                 }
-                if (!PATH55) gD[r * pf] = divp;
+                if (!PATH55) bD[of + r * pf] = divp;
             }
         }
     }
@@ -540,9 +540,10 @@ struct Tiled {
                 tmem_st<4>(tdl + r * TBLOCK + FXYCOL, r4);
             }
         }
-        const long long plane_w = (long long)g.nx * g.ny, plane_f = (long long)g.px * g.py;
-        long long ow = ci + (long long)g.nx * (cj + (long long)g.ny * zs);
-        long long of = (ci + g.gx) + (long long)g.px * ((cj + g.gy) + (long long)g.py * (zs + g.gz));
+        const uint32_t plane_w = (uint32_t)g.nx * g.ny, plane_f = (uint32_t)g.px * g.py;
+        // 32-bit element offsets (tiled_supported guarantees 4 fs, 4 n < 2^32): one wide multiply-add per store address
+        uint32_t ow = (uint32_t)(ci + (long long)g.nx * (cj + (long long)g.ny * zs));
+        uint32_t of = (uint32_t)((ci + g.gx) + (long long)g.px * ((cj + g.gy) + (long long)g.py * (zs + g.gz)));
         if (!store_ok) { ow = 0; of = 0; }
         State st[RY];
 #pragma unroll
@@ -570,7 +571,7 @@ struct Tiled {
                     mbar_wait(a_full + 8 * (ph & (NS - 1)), (uint32_t)((p >> LNS) & 1));
                     if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
 #define FD6_STEP(K) \
-    step<K>(st, sp0, wsp0, tdl, c, out, Fout + of, W + ow, Div + of, g.fs, g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R))
+    step<K>(st, sp0, wsp0, tdl, c, out, Fout, W, Div, of, ow, (uint32_t)g.fs, (uint32_t)g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R))
                     switch (ph) {  // ph is a compile-time constant after unrolling
                         case 0: FD6_STEP(0); break;
                         case 1: FD6_STEP(1); break;
@@ -658,7 +659,9 @@ struct TiledState {
     char err[256] = "";
 };
 
-inline bool tiled_supported(const Geom& g) { return g.nx >= 4 && g.ny >= 4 && g.nz >= 4; }
+inline bool tiled_supported(const Geom& g) {  // the kernels address F_out and w with 32-bit element offsets
+    return g.nx >= 4 && g.ny >= 4 && g.nz >= 4 && 4 * g.fs < (1LL << 32) && 4 * g.n < (1LL << 32);
+}
 
 inline PFN_encodeTiled tiled_encode_fn() {
     static PFN_encodeTiled fn = nullptr;
