@@ -515,7 +515,10 @@ struct Tiled {
             __syncthreads();
         }
         // a warp reaches the 32 lanes of its quadrant (warp % 4); warps that share a quadrant use different columns
-        const uint32_t tdl = tmem_base + ((uint32_t)(((tid >> 5) & 3) * 32) << 16) + (uint32_t)((tid >> 7) * RY * TBLOCK);
+        // (the address is the same for all lanes of a warp; the warp-wide OR tells the compiler so: it then lives in a
+        // uniform register for the whole loop instead of being re-derived and moved there before every tcgen05 access)
+        const uint32_t tdl =
+            __reduce_or_sync(0xffffffffu, tmem_base + ((uint32_t)(((tid >> 5) & 3) * 32) << 16) + (uint32_t)((tid >> 7) * RY * TBLOCK));
         if (producer) {
             for (int i = 0; i < NS && i < np; ++i) {
                 mbar_expect_tx(a_full + 8 * i, kStageBytes);
