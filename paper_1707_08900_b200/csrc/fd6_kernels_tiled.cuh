@@ -464,7 +464,7 @@ struct Tiled {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
         T* smw = sm + NS * STAGE;
-        const uint32_t a_sm = smem_u32(smem_raw);
+        const uint32_t a_sm = __reduce_or_sync(0xffffffffu, smem_u32(smem_raw));  // uniform: kept in a uniform register
         const uint32_t a_smw = a_sm + (uint32_t)(NS * STAGE * sizeof(T));
         const uint32_t a_full = a_smw + (uint32_t)(NW * WSTAGE * sizeof(T)), a_empty = a_full + 8 * NS, a_wfull = a_empty + 8 * NS;
         const int tx = threadIdx.x, ty = threadIdx.y;
