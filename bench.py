@@ -37,8 +37,8 @@ WORDS_PER_CELL_SUBSTEP = {"55": 16, "19": 30}  # SURVEY.md 8(d), DESIGN.md "Kern
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel at C4, from the committed
 # `ncu --set full` capture (profiles/); None until that capture exists for the kernel bench.py times.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_ncu_fused55_paired_v7_C4.md, launch B (the substep that reads and writes w)
-    ("C4", "fused55"): 8.846e9,
+    # profiles/r01_ncu_fused55_paired_v8_C4.md, launch B (the substep that reads and writes w)
+    ("C4", "fused55"): 8.838e9,
 }
 
 
