@@ -123,3 +123,21 @@ def test_forced_c4_512_fp32_sampled_blocks(mods):
         got = I.gather_block(out, tuple(o + m for o in origin), inner)
         worst = max(worst, relinf(got, ref))
     assert worst <= TOL["f32"]
+
+
+def test_forcing_argument_errors_on_a_live_context(mods):
+    O, fd6, I = mods
+    ctx = fd6.Fd(32, 32, 32, 0.2, 0.01, 1.0, fd6.FD_F32)
+    for args in [((0, 0, 2), (0, 0, 1), 0.0, 1.0, 0.01),        # k parallel to e
+                 ((1, 0, 0), (0, 1, 0), 0.0, -1.0, 0.01),       # f0 < 0
+                 ((1, 0, 0), (0, 1, 0), 0.0, 1.0, 0.0),         # dt_ref <= 0
+                 ((1, 0, 0), (0, 1, 0), float("nan"), 1.0, 0.01),
+                 ((float("inf"), 0, 0), (0, 1, 0), 0.0, 1.0, 0.01),
+                 (None, None, 0.0, 1.0, 0.01)]:                  # NULL vectors with f0 != 0
+        with pytest.raises(fd6.FdError) as ei:
+            ctx.fd_set_forcing(*args)
+        assert ei.value.code == fd6.FD_EINVAL
+    ctx.fd_set_forcing(None, None, 0.0, 0.0, 1.0)  # switching off needs no vectors
+    ctx.fd_rk3_step(0.01, 1)                       # and a failed call left the context usable
+    assert np.array_equal(ctx.store_state(), np.zeros((4, 32, 32, 32), np.float32))
+    ctx.fd_destroy()
