@@ -368,3 +368,26 @@ def test_paired_variant_is_refused_where_it_cannot_run(mods):
         ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)
     assert e.value.code == fd6.FD_EUNSUPPORTED
     ctx.fd_destroy()
+
+
+# ------------------------------------------------- work-list corners: many tiles, few planes; ragged everything
+@pytest.mark.parametrize("shape,dtype", [((512, 500, 16), "f32"), ((512, 500, 16), "f64"), ((1024, 300, 8), "f32"),
+                                         ((36, 1000, 10), "f64"), ((2048, 100, 9), "f32"), ((132, 2000, 12), "f32")])
+@pytest.mark.parametrize("path", [0, 1])
+def test_many_tiles_few_planes(mods, shape, dtype, path):
+    """Grids whose tile count exceeds the SM count (full columns AND a z-chunked remainder in one launch) with very
+    few planes, odd plane counts (plain fp32 layout) and ragged tiles, one step against the oracle on the full grid."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(11)
+    dx, nu, cs = 0.1, 0.004, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.05, dtype)
+    ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32 if dtype == "f32" else fd6.FD_F64)
+    ctx.fd_set_path(path)
+    wl = fd6.fd_plan_work_list(*shape, fd6.FD_F32 if dtype == "f32" else fd6.FD_F64, 148)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(dt, 1)
+    got = ctx.store_state()
+    ctx.fd_destroy()
+    ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 1, path)
+    assert relinf(got, ref) <= TOL[dtype], (wl.full_tiles, wl.chunks, wl.chunk_planes, wl.items)
