@@ -297,7 +297,12 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         if (rc) return rc;
         if (tiled) s.dt = T(typename Scalar<T>::type(1));  // the tiled pass 1 leaves dt * div u in Div
         LaunchScope ls(c, FD_K_PASS2);
-        k_direct_pass2<T><<<grid, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+        // y bands of 16 block rows once seven div planes no longer fit comfortably in L2 (see k_direct_pass2)
+        const int brows = (g.ny + 3) / 4;
+        const bool banded = 7.0 * g.px * g.py * (double)c->esize > 32e6 && brows > 16;
+        const int band_rows = banded ? 16 : brows, bands = (brows + band_rows - 1) / band_rows;
+        dim3 grid2((g.nx + 63) / 64, band_rows, bands * g.nz);
+        k_direct_pass2<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
     }
     FD_CUDA(cudaGetLastError());
     if (s.write_f) {
