@@ -148,11 +148,6 @@ int fd_set_profiling(fd_ctx* ctx, int on);
 int fd_get_profile(fd_ctx* ctx, int kernel_id, double* total_ms, unsigned long long* launches);
 int fd_reset_profile(fd_ctx* ctx);
 
-/* Test hooks: overwrite the w arrays / every ghost cell of both field copies with a quiet NaN, to prove that
- * neither stale w (alpha_1 = 0) nor stale ghosts can reach a result. */
-int fd_debug_poison_w(fd_ctx* ctx);
-int fd_debug_poison_ghosts(fd_ctx* ctx);
-
 #ifdef __cplusplus
 }
 #endif

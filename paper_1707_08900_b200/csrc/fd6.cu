@@ -2,6 +2,7 @@
 // Every step of the path runs in the kernels of fd6_kernels_*.cuh; this file only allocates, orders
 // launches on the context's stream and swaps pointers.
 #include "../../include/fd6.h"
+#include "../../include/fd6_testing.h"
 
 #include <cmath>
 #include <cstdarg>
@@ -461,27 +462,44 @@ static int set_layout(fd_ctx* c, bool paired) {
     return rc;
 }
 
+// Pick the kernel variant and bring layout, tensor maps and work list in line with it.  Nothing is changed
+// unless the whole switch succeeds: an unsupported target is refused before the layout is touched, and if the
+// tensor-map setup fails afterwards the previous layout and variant are restored (c->variant, c->paired and
+// c->tiled always describe the same kernels).
 static int resolve_variant(fd_ctx* c) {
     int want = c->variant_req;
-    if (want == FD_VARIANT_AUTO) want = pair_ok(c) ? FD_VARIANT_PAIRED : FD_VARIANT_TILED;
-    if (want == FD_VARIANT_PAIRED && !pair_ok(c)) {
-        if (c->variant_req != FD_VARIANT_AUTO)
-            return fail(FD_EUNSUPPORTED, "paired variant needs fp32 and an even nz >= 8 (got dtype %d, nz %d)", c->dtype, c->nz);
-        want = FD_VARIANT_TILED;
-    }
-    // layout: the paired variant needs the paired layout, the plain tiled one the plain layout; direct runs on either
-    int rc = FD_OK;
-    if (want == FD_VARIANT_PAIRED) rc = set_layout(c, true);
-    if (want == FD_VARIANT_TILED) rc = set_layout(c, false);
-    if (rc) return rc;
+    const bool is_auto = want == FD_VARIANT_AUTO;
+    if (is_auto) want = pair_ok(c) ? FD_VARIANT_PAIRED : FD_VARIANT_TILED;
+    if (want == FD_VARIANT_PAIRED && !pair_ok(c))
+        return fail(FD_EUNSUPPORTED, "paired variant needs fp32 and an even nz >= 8 (got dtype %d, nz %d)", c->dtype, c->nz);
     if (want == FD_VARIANT_TILED || want == FD_VARIANT_PAIRED) {
-        rc = tiled_supported(c->g) ? FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W)) : 4;
+        const bool tp = want == FD_VARIANT_PAIRED;
+        const Geom tg = make_geom(c->nx, c->ny, c->nz, tp ? 8 : (c->dtype == FD_F32 ? 4 : 8), tp);
+        if (!tiled_supported(tg)) {  // checked on the TARGET layout, before anything is converted
+            if (!is_auto)
+                return fail(FD_EUNSUPPORTED,
+                            "tiled variant cannot run this grid in the %s layout: it needs >= 4 values per axis and "
+                            "4 * padded field size < 2^32 values (the kernels use 32-bit store offsets)", tp ? "paired" : "plain");
+            want = FD_VARIANT_DIRECT;
+        }
+    }
+    if (want == FD_VARIANT_TILED || want == FD_VARIANT_PAIRED) {
+        const bool was_paired = c->paired;
+        const int was_variant = c->variant;
+        int rc = set_layout(c, want == FD_VARIANT_PAIRED);
+        if (rc) return rc;
+        rc = FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W));
         if (rc != FD_OK) {
-            if (c->variant_req == FD_VARIANT_AUTO) {
-                want = FD_VARIANT_DIRECT;
+            char why[256];
+            snprintf(why, sizeof(why), "%s", tiled_error_of(c->tiled));
+            if (is_auto) {
+                want = FD_VARIANT_DIRECT;  // runs on either layout
             } else {
-                return fail(rc == 4 ? FD_EUNSUPPORTED : FD_ECUDA, "tiled variant setup failed: %s",
-                            rc == 4 ? "grid too small" : tiled_error_of(c->tiled));
+                int rb = set_layout(c, was_paired);
+                if (rb == FD_OK && (was_variant == FD_VARIANT_TILED || was_variant == FD_VARIANT_PAIRED))
+                    rb = FD_DISPATCH(c, tiled_prepare<T>(c->tiled, c->g, c->F[0], c->F[1], c->W));
+                if (rb != FD_OK) c->variant = FD_VARIANT_DIRECT;  // last resort: the direct kernels need no setup
+                return fail(FD_ECUDA, "tiled variant setup failed: %s", why);
             }
         }
     }
@@ -807,6 +825,7 @@ static int do_poison(fd_ctx* c, bool ghosts) {
     return FD_OK;
 }
 
+// ---- include/fd6_testing.h: test hooks, not part of the product ABI ----
 extern "C" int fd_debug_poison_w(fd_ctx* c) {
     FD_CHECK_CTX(c);
     return FD_DISPATCH(c, do_poison<T>(c, false));

@@ -24,7 +24,7 @@ KERNEL_NAMES = ["pack", "unpack", "halo", "fused55", "pass1_19", "pass2_19"]
 EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
     "fd_rhs", "fd_rk3_step", "fd_sync", "fd_destroy", "fd_last_error", "fd_get_info", "fd_kernel_launches",
-    "fd_set_profiling", "fd_get_profile", "fd_reset_profile", "fd_debug_poison_w", "fd_debug_poison_ghosts",
+    "fd_set_profiling", "fd_get_profile", "fd_reset_profile",
     "fd_plan_work_list", "fd_set_forcing",
 ]
 
@@ -70,8 +70,6 @@ lib.fd_kernel_launches.restype = C.c_ulonglong
 lib.fd_set_profiling.argtypes = [_vp, _i]
 lib.fd_get_profile.argtypes = [_vp, _i, C.POINTER(_d), C.POINTER(C.c_ulonglong)]
 lib.fd_reset_profile.argtypes = [_vp]
-lib.fd_debug_poison_w.argtypes = [_vp]
-lib.fd_debug_poison_ghosts.argtypes = [_vp]
 lib.fd_set_forcing.argtypes = [_vp, C.POINTER(_d), C.POINTER(_d), _d, _d, _d]
 lib.fd_plan_work_list.argtypes = [_i, _i, _i, _i, _i, C.POINTER(FdWorkList)]
 
@@ -206,14 +204,6 @@ class Fd:
 
     def fd_reset_profile(self):
         _check(lib.fd_reset_profile(self._h))
-
-    def fd_debug_poison_w(self):
-        self._stream()
-        _check(lib.fd_debug_poison_w(self._h))
-
-    def fd_debug_poison_ghosts(self):
-        self._stream()
-        _check(lib.fd_debug_poison_ghosts(self._h))
 
     def fd_destroy(self):
         if self._h:

@@ -17,8 +17,8 @@ def fd6():
     return mod
 
 
-def declared_functions():
-    src = open(os.path.join(ROOT, "include", "fd6.h")).read()
+def declared_functions(header="fd6.h"):
+    src = open(os.path.join(ROOT, "include", header)).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
     return sorted(set(re.findall(r"\b(fd_[a-z0-9_]+)\s*\(", src)) - {"fd_alloc_fn", "fd_free_fn"})
 
@@ -33,6 +33,25 @@ def test_library_exports_every_declared_symbol(fd6):
     for name in declared_functions():
         assert hasattr(fd6.lib, name), f"libfd6.so does not export {name}"
     assert sorted(fd6.EXPORTS) == declared_functions()
+
+
+def test_test_hooks_live_in_their_own_header(fd6):
+    """include/fd6.h is the product ABI; the NaN-poison hooks are declared in include/fd6_testing.h only."""
+    from paper_1707_08900_b200 import fd6_testing
+    hooks = declared_functions("fd6_testing.h")
+    assert hooks == sorted(fd6_testing.TEST_EXPORTS) and hooks
+    assert not set(hooks) & set(declared_functions())
+    assert not any("debug" in n for n in declared_functions())
+    for name in hooks:
+        assert hasattr(fd6.lib, name), f"libfd6.so does not export {name}"
+
+
+def test_every_dynamic_fd_symbol_is_declared_in_a_header(fd6):
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", os.path.join(ROOT, "paper_1707_08900_b200", "libfd6.so")],
+                         capture_output=True, text=True).stdout
+    syms = sorted({ln.split()[-1] for ln in out.splitlines() if ln.split() and ln.split()[-1].startswith("fd_")})
+    assert syms == sorted(declared_functions() + declared_functions("fd6_testing.h"))
 
 
 def test_library_does_not_link_torch_or_the_oracle(fd6):

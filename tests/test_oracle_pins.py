@@ -555,6 +555,18 @@ def test_p12_float_instantiation_tracks_double():
     assert relinf(b.astype(np.float64), a) < 2e-6
 
 
+@pytest.mark.parametrize("path", [P55, P19])
+def test_p12_float_rhs_tracks_double(path):
+    """fdo_rhs_f32 (the float instantiation of the pinned template) follows fdo_rhs_f64 on fp32-representable inputs."""
+    cfg = I.CONFIGS["C2"]
+    F32 = I.make_state(cfg, n_override=24)
+    dx = TWO_PI / 24
+    a = O.rhs(F32.astype(np.float64), dx, cfg.nu, cfg.cs, path)
+    b = O.rhs(F32, dx, cfg.nu, cfg.cs, path, dtype=np.float32)
+    assert b.dtype == np.float32
+    assert relinf(b.astype(np.float64), a) < 2e-6
+
+
 # ------------------------------------------------------------------------------------------------------------------
 # P13  forcing term of Eq. 2 (Eq. 24-25, PAPER.md:425-429; SURVEY 8(f)-2, oracle step O11)
 def _forcing_expected(spec, cs):

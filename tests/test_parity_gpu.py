@@ -7,6 +7,8 @@ import math
 import numpy as np
 import pytest
 
+from paper_1707_08900_b200 import fd6_testing as T  # include/fd6_testing.h: NaN-poison hooks (tests only)
+
 pytestmark = pytest.mark.gpu
 
 TOL = {"f64": 1e-12, "f32": 2e-5}
@@ -99,7 +101,7 @@ def test_c1_one_step_and_rhs_full_grid_fp64(mods, path, variant):
     R = ctx.rhs_state()
     assert relinf(R, O.rhs(F, cfg.dx, cfg.nu, cfg.cs, path)) <= TOL["f64"]
     assert np.array_equal(ctx.store_state(), F)  # fd_rhs leaves the state untouched
-    ctx.fd_debug_poison_w()                        # stale w must not matter: alpha^(1) = 0
+    T.fd_debug_poison_w(ctx)                        # stale w must not matter: alpha^(1) = 0
     ctx.fd_rk3_step(cfg.dt, 1)
     got = ctx.store_state()
     ref = O.rk3_step(F, cfg.dx, cfg.nu, cfg.cs, cfg.dt, 1, path)
@@ -119,7 +121,7 @@ def test_ragged_grids_three_steps(mods, shape, dtype, path, variant):
     dt = 0.1 * dx
     F = smooth_state(rng, shape, 0.1, dtype)
     ctx = make_ctx(fd6, shape, dx, nu, cs, dtype, path, variant)
-    ctx.fd_debug_poison_ghosts()  # every ghost that is read must have been filled by the library
+    T.fd_debug_poison_ghosts(ctx)  # every ghost that is read must have been filled by the library
     ctx.load_state(F)
     ctx.fd_rk3_step(dt, 1)
     one = ctx.store_state()
@@ -220,7 +222,7 @@ def _sample_origins(n, size, rng, extra):
     return pts
 
 
-def _windowed_check(mods, cfg_name, path, variant, n_override=None, inner=16, nblocks=8):
+def _windowed_check(mods, cfg_name, path, variant, n_override=None, inner=16, nblocks=8, before_step=None):
     import torch
     O, fd6, I = mods
     cfg = I.CONFIGS[cfg_name]
@@ -230,6 +232,8 @@ def _windowed_check(mods, cfg_name, path, variant, n_override=None, inner=16, nb
     F = I.make_state(cfg, device="cuda", n_override=n_override)
     ctx = make_ctx(fd6, (n,) * 3, dx, cfg.nu, cfg.cs, cfg.dtype, path, variant)
     ctx.load_state(F)
+    if before_step:
+        before_step(ctx)
     ctx.fd_rk3_step(dt, 1)
     out = torch.empty_like(F)
     ctx.store_state(out)
@@ -268,7 +272,18 @@ def test_c5_1024_fp32_sampled_blocks(mods, path):
     free, _ = torch.cuda.mem_get_info()
     if free < 90e9:
         pytest.skip("needs ~80 GB of free device memory")
-    assert _windowed_check(mods, "C5", path, 0, nblocks=6) <= TOL["f32"]
+    fd6 = mods[1]
+
+    def rejected_switch(ctx):
+        """The plain-layout tiled kernel cannot address 1024^3 (32-bit store offsets): an explicit request is refused
+        BEFORE anything is converted, and the context keeps stepping with the variant it had."""
+        assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED
+        with pytest.raises(fd6.FdError) as e:
+            ctx.fd_set_variant(fd6.FD_VARIANT_TILED)
+        assert e.value.code == fd6.FD_EUNSUPPORTED and "2^32" in str(e.value)
+        assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED
+
+    assert _windowed_check(mods, "C5", path, 0, nblocks=6, before_step=rejected_switch if path == 0 else None) <= TOL["f32"]
 
 
 def test_c3_256_fp64_full_grid_55(mods):
