@@ -286,7 +286,7 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
                                         c->force_on ? c->famp : no_force);
             const int lrc = tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, ft, c->stream);
             if (lrc == 4) return fail(FD_EUNSUPPORTED, "forcing on a grid with this many planes needs FD_VARIANT_DIRECT");
-            if (lrc) return fail(FD_ECUDA, "tiled kernel launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+            if (lrc) return fail(FD_ECUDA, "tiled kernel launch failed: %s", tiled_error_of(c->tiled));
         } else if (p55) {
             k_direct_main<T, true><<<grid, block, 0, c->stream>>>(Fin, Fout, W, nullptr, g, k, s, ft);
         } else {

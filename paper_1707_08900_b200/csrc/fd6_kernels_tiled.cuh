@@ -30,6 +30,8 @@
 #pragma once
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "fd6_common.cuh"
 
 namespace fd6 {
@@ -136,6 +138,42 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t* r) {
         : "r"(taddr)
         : "memory");
 }
+// Results of tcgen05.ld may be used only after tcgen05.wait::ld.  The *_nc variants carry no "memory" clobber (so the
+// compiler may move shared-memory loads across them; volatile asm statements keep their order among themselves);
+// instead the loaded registers are passed through tmem_fence*, an empty volatile asm placed after the wait, so that
+// every consumer depends on it.
+__device__ __forceinline__ void tmem_ld16_nc(uint32_t taddr, uint32_t* r) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld8_nc(uint32_t taddr, uint32_t* r) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+                 : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_ld4_nc(uint32_t taddr, uint32_t* r) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st2_nc(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]));
+}
+__device__ __forceinline__ void tmem_st8_nc(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]),
+                 "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]));
+}
+__device__ __forceinline__ void tmem_st4_nc(uint32_t taddr, const uint32_t* r) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]));
+}
+__device__ __forceinline__ void tmem_wait_ld_nc() { asm volatile("tcgen05.wait::ld.sync.aligned;"); }
+__device__ __forceinline__ void tmem_wait_st_nc() { asm volatile("tcgen05.wait::st.sync.aligned;"); }
+__device__ __forceinline__ void tmem_fence16(uint32_t* r) {
+    asm volatile("" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3]), "+r"(r[4]), "+r"(r[5]), "+r"(r[6]), "+r"(r[7]), "+r"(r[8]), "+r"(r[9]),
+                      "+r"(r[10]), "+r"(r[11]), "+r"(r[12]), "+r"(r[13]), "+r"(r[14]), "+r"(r[15]));
+}
+__device__ __forceinline__ void tmem_fence4(uint32_t* r) { asm volatile("" : "+r"(r[0]), "+r"(r[1]), "+r"(r[2]), "+r"(r[3])); }
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 // six values of T <-> 6 * sizeof(T) / 4 registers
@@ -193,16 +231,20 @@ struct Regs6 {
 
 // TX x TY threads; a thread owns RY vertically adjacent columns (rows cj .. cj+RY-1), so the tile is TX x (TY*RY).
 // FORCE: the forcing term of Eq. 2 is added (a separate instantiation, so the unforced kernel pays nothing).
-template <class T, bool PATH55, int TX, int TY, int NS_, int RY, bool FORCE>
+// MODE: what the RK update of the launch touches, known at compile time so that the plane loop holds no runtime
+// predicates on it: bit 0 = w is read (alpha != 0), bit 1 = w is written, bit 2 = F_out is written.  The four modes
+// in use: 6 = substep 1 (alpha_1 = 0: w not read), 7 = substep 2, 5 = substep 3 (its w is never read again: not
+// written), 2 = fd_rhs (w <- rhs only).
+template <class T, bool PATH55, int TX, int TY, int NS_, int RY, bool FORCE, int MODE>
 struct Tiled {
+    static constexpr bool RW = (MODE & 1) != 0, WW = (MODE & 2) != 0, WF = (MODE & 4) != 0;
     static constexpr int TH = TY * RY;  // tile height in values
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
     static constexpr int PYS = TH + 2 * R;
     static constexpr int FIELD = PXS * PYS;
     static constexpr int STAGE = 4 * FIELD;  // values per stage: four fields of one plane
     static constexpr int NS = NS_;           // stages (4 or 8); the plane loop is unrolled 8x, so stage offsets are immediates
-    static_assert(NS == 4 || NS == 8, "ring depth");
-    static constexpr int LNS = NS == 8 ? 3 : 2;
+    static_assert(NS == 4, "ring depth: the producer requests plane p + 3 and the w tile of the same iteration on one barrier");
     static constexpr int NW = 4;             // w stages
     static constexpr int WFIELD = TX * TH;
     static constexpr int WSTAGE = 4 * WFIELD;
@@ -220,7 +262,7 @@ struct Tiled {
     static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * RY * TBLOCK;
     static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
     static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
-    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 2) * sizeof(uint64_t);
+    static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + 2) * sizeof(uint64_t);
     static size_t smem_bytes(int planes) { return SMEM + (FORCE ? 2 * (size_t)planes * sizeof(T) : 0); }  // + the z table
     static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
@@ -233,7 +275,7 @@ struct Tiled {
     // scatter of the in-plane differences e_m of plane t into the accumulator ring of one rhs component (Eq. 8 with z)
     template <int n8>
     static __device__ __forceinline__ void scatter(T (&lin)[8], const T (&e)[3], const KC<T>& c) {
-        lin[(n8 + 3) & 7] = -(c.mq[2] * e[2]);  // first contribution to output t+3
+        lin[(n8 + 3) & 7] = (-c.mq[2]) * e[2];  // first contribution to output t+3 (the sign goes with the constant: free)
         lin[(n8 + 2) & 7] = fma_(-c.mq[1], e[1], lin[(n8 + 2) & 7]);
         lin[(n8 + 1) & 7] = fma_(-c.mq[0], e[0], lin[(n8 + 1) & 7]);
         lin[(n8 + 7) & 7] = fma_(c.mq[0], e[0], lin[(n8 + 7) & 7]);
@@ -241,22 +283,69 @@ struct Tiled {
         lin[(n8 + 5) & 7] = fma_(c.mq[2], e[2], lin[(n8 + 5) & 7]);  // output t-3 is complete
     }
 
-    // One plane.  sp0: the thread's first centre in stage 0 of the F ring; wsp0: its first element in stage 0 of the
-    // w ring; bF, bW, bD + of / ow: its first cell of output plane z = t - 3 in F_out, w and div (field strides fs, n; row
-    // pitches pf, pw); `out`: that plane is produced; ok[r]: owned column r lies inside the grid.  FORCE: ftz points
-    // at (cos, sin) of k_z z of the output plane in shared memory; cos and sin of k_x x + k_y y + phi of the owned
-    // columns sit in four spare tensor-memory columns (8-byte types) or are re-read from the tables ft (plain fp32).
+    // Output plane z = t - 4, field f of one owned column: centre value, D1z and (u fields) D2z + the finished
+    // accumulator, from the window ring (slot t = n8 is not among the seven used).  wr: the ring of field f as fetched
+    // from tensor memory (after tcgen05.wait::ld); plain fp32: the ring is st.win[f] and slot t is rewritten with cnew.
+    template <int n8>
+    static __device__ __forceinline__ void zfield(int f, State& st, uint32_t (&wr)[16], T cnew, T (&fc)[4], T (&d1z)[4], T (&lz)[3], const KC<T>& c) {
+        constexpr int cz = (n8 + 4) & 7;
+        T w8[8];
+        if constexpr (TM) {
+            tmem_fence16(wr);
+#pragma unroll
+            for (int a8 = 0; a8 < 8; ++a8) {
+                const uint2 u = make_uint2(wr[2 * a8], wr[2 * a8 + 1]);
+                w8[a8] = *reinterpret_cast<const T*>(&u);
+            }
+        } else {
+#pragma unroll
+            for (int a8 = 0; a8 < 8; ++a8) w8[a8] = st.win[f][a8];
+            st.win[f][n8] = cnew;  // after the read: slot t is unused by this output
+        }
+        const T* a = f == 0 ? c.ar : c.au;
+        fc[f] = w8[cz];
+        d1z[f] = fma_(a[2], w8[(cz + 3) & 7] - w8[(cz + 5) & 7], fma_(a[1], w8[(cz + 2) & 7] - w8[(cz + 6) & 7], a[0] * (w8[(cz + 1) & 7] - w8[(cz + 7) & 7])));
+        if (f > 0) {
+            const T* bz = f == 3 ? c.lq : c.lo;
+            T v = fma_(bz[0], fc[f], st.lin[f - 1][cz]);
+            v = fma_(bz[1], w8[(cz + 1) & 7] + w8[(cz + 7) & 7], v);
+            v = fma_(bz[2], w8[(cz + 2) & 7] + w8[(cz + 6) & 7], v);
+            v = fma_(bz[3], w8[(cz + 3) & 7] + w8[(cz + 5) & 7], v);
+            lz[f - 1] = v;
+        }
+    }
+
+    // ---- One iteration of the software-pipelined plane loop ---------------------------------------------------
+    // In-plane work of plane t AND the output of plane z = t - 4 in ONE basic block.  The output lags the load front by
+    // four planes instead of three: output z needs planes z-3 .. z+3 (all consumed in earlier iterations), so nothing
+    // in the output part depends on the in-plane part of the same iteration and the compiler may interleave them:
+    //   lin ring   in-plane(t) scatters into slots t-3 .. t+3; output reads slot t-4 = t+4 (mod 8): all 8 slots live
+    //   window     in-plane(t) writes slot t; output reads the 7 other slots
+    //   delay line slot t & 3 is read (plane t-4) BEFORE it is rewritten with the values of plane t
+    //   w ring     output index q = p - 7 uses slot q & 3
+    // RY == 1: the output side of field f follows the in-plane side of field f, so that its arithmetic fills the gaps
+    // between the shared-memory loads of the next field (SPLIT = false).  RY > 1: the output side runs column by
+    // column after the in-plane side, which keeps fewer values live at once (SPLIT = true).
+    // `out` only gates the stores (warm-up iterations compute on zero-initialised state and store nothing).
+    static constexpr bool SPLIT = RY > 1;
     template <int PH>
-    static __device__ __forceinline__ void step(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
-                                                const KC<T>& c, bool out, T* __restrict__ bF, T* __restrict__ bW, T* __restrict__ bD, uint32_t of, uint32_t ow,
-                                                uint32_t fs, uint32_t n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
+    static __device__ __forceinline__ void plane(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
+                                                 const KC<T>& c, bool out, T* __restrict__ bF, T* __restrict__ bW, T* __restrict__ bD, uint32_t of, uint32_t ow,
+                                                 uint32_t fs, uint32_t n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
-        const T* sp = sp0 + (PH & (NS - 1)) * STAGE;
-        // ---- plane t: in-plane derivatives of the four fields (Eq. 6-8).  The RY + 6 values of the thread's own
-        // x column are loaded once per field and serve the y stencils of all its outputs.
+        const T* sp = sp0 + (PH & 3) * STAGE;
+        const T* wsp = wsp0 + ((PH + 1) & 3) * WSTAGE;  // w ring slot of output index p - 7
         T ctr[RY][4], d1x[RY][4], d1y[RY][4], inpl[RY][3], ezx[RY][3];
+        T fc[RY][4], d1z[RY][4], lz[RY][3];
+        uint32_t wr[RY][16];
+        if constexpr (TM && !SPLIT) {
+#pragma unroll
+            for (int r = 0; r < RY; ++r) tmem_ld16_nc(tdl + r * TBLOCK + TWIN, wr[r]);
+        }
 #pragma unroll
         for (int f = 0; f < 4; ++f) {
+            // ---- plane t, field f: in-plane derivatives (Eq. 6-8).  The RY + 6 values of the thread's own x column are
+            // loaded once per field and serve the y stencils of all its outputs.
             const T* q0 = sp + f * FIELD;
             T yv[RY + 2 * R];
 #pragma unroll
@@ -268,9 +357,7 @@ struct Tiled {
                 if constexpr (TM) {
                     const uint2 u = *reinterpret_cast<const uint2*>(&ctr[r][f]);
                     const uint32_t r2[2] = {u.x, u.y};
-                    tmem_st<2>(tdl + r * TBLOCK + TWIN + f * 16 + n8 * 2, r2);
-                } else {
-                    st[r].win[f][n8] = ctr[r][f];
+                    tmem_st2_nc(tdl + r * TBLOCK + TWIN + f * 16 + n8 * 2, r2);
                 }
                 const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
                 const T yp1 = yv[r + R + 1], ym1 = yv[r + R - 1], yp2 = yv[r + R + 2], ym2 = yv[r + R - 2], yp3 = yv[r + R + 3], ym3 = yv[r + R - 3];
@@ -314,8 +401,26 @@ struct Tiled {
                     }
                 }
             }
+            if constexpr (!SPLIT) {  // output side of field f right here
+                if constexpr (TM) tmem_wait_ld_nc();
+#pragma unroll
+                for (int r = 0; r < RY; ++r) zfield<n8>(f, st[r], wr[r], ctr[r][f], fc[r], d1z[r], lz[r], c);
+                if constexpr (TM) {
+                    if (f < 3) {
+#pragma unroll
+                        for (int r = 0; r < RY; ++r) tmem_ld16_nc(tdl + r * TBLOCK + TWIN + (f + 1) * 16, wr[r]);
+                    }
+                }
+            }
+        }
+        // the delayed in-plane values of plane t - 4 (slot t & 3, read before it is rewritten below)
+        uint32_t dr[RY][16];
+        if constexpr (TM && !SPLIT) {
+#pragma unroll
+            for (int r = 0; r < RY; ++r) tmem_ld16_nc(tdl + r * TBLOCK + n4 * DLCOLS, dr[r]);  // 12 values + 4 spare columns
         }
         // ---- plane t: everything of dt*rhs that needs no z derivative (Eq. 1-3); G' = dt * grad u
+        T park[RY][6];
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
             const T gx = d1x[r][0], gy = d1y[r][0], ux = ctr[r][1], uy = ctr[r][2];
@@ -345,77 +450,45 @@ struct Tiled {
                 else
                     st[r].lin[i][n8] = pl[i];
             }
-            // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of plane t -> delay-line slot t & 3
-            if constexpr (TM) {
-                const T park[6] = {gx, gy, Gzx, Gzy, Dh, P0};
-                Regs6<T>::store(tdl + r * TBLOCK + n4 * DLCOLS, park);
-            } else {
-                st[r].dl[0][n4] = gx;
-                st[r].dl[1][n4] = gy;
-                st[r].dl[2][n4] = Gzx;
-                st[r].dl[3][n4] = Gzy;
-                st[r].dl[4][n4] = Dh;
-                st[r].dl[5][n4] = P0;
-            }
+            park[r][0] = gx; park[r][1] = gy; park[r][2] = Gzx; park[r][3] = Gzy; park[r][4] = Dh; park[r][5] = P0;
         }
-        if (!out) return;
-        // ---- output plane z = t - 3: z derivatives from the window, the rest of Eq. 1-3, Eq. 10
-        constexpr int cz = (n8 + 5) & 7, r4 = (n4 + 1) & 3;
-        const T* wsp = wsp0 + ((PH + 2) & 3) * WSTAGE;  // w ring slot of plane index p - 6
+        if constexpr (TM && !SPLIT) tmem_wait_ld_nc();
+        // ---- output plane z = t - 4: the rest of Eq. 1-3, Eq. 10
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
-            T d1z[4], fc[4], del[6];
-            uint32_t fr[4];  // FORCE && TM: cos, sin of the xy phase of the owned column, from tensor memory
-            if constexpr (TM) {
-                // the whole window ring of a field is 16 consecutive columns: one load each; slot t of this plane may
-                // still be in flight, so it is taken from the register that holds it
-                uint32_t wr[4][16], dr[12];
+            if constexpr (SPLIT) {  // the whole output side of this column: window rings and delay line in one batch
+                uint32_t w4[4][16];
+                if constexpr (TM) {
 #pragma unroll
-                for (int f = 0; f < 4; ++f) tmem_ld16(tdl + r * TBLOCK + TWIN + f * 16, wr[f]);
-                tmem_ld<8>(tdl + r * TBLOCK + r4 * DLCOLS, dr);
-                tmem_ld<4>(tdl + r * TBLOCK + r4 * DLCOLS + 8, dr + 8);
-                if constexpr (FORCE && !FXY_LATE) tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr);
-                tmem_wait_ld();
-#pragma unroll
-                for (int f = 0; f < 4; ++f) {
-#pragma unroll
-                    for (int a8 = 0; a8 < 8; ++a8) {
-                        const uint2 u = make_uint2(wr[f][2 * a8], wr[f][2 * a8 + 1]);
-                        st[r].win[f][a8] = *reinterpret_cast<const T*>(&u);
-                    }
-                    st[r].win[f][n8] = ctr[r][f];
+                    for (int f = 0; f < 4; ++f) tmem_ld16_nc(tdl + r * TBLOCK + TWIN + f * 16, w4[f]);
+                    tmem_ld16_nc(tdl + r * TBLOCK + n4 * DLCOLS, dr[r]);
+                    tmem_wait_ld_nc();
                 }
-                Regs6<T>::unpack(dr, del);
+#pragma unroll
+                for (int f = 0; f < 4; ++f) zfield<n8>(f, st[r], w4[f], ctr[r][f], fc[r], d1z[r], lz[r], c);
+            }
+            T del[6];
+            if constexpr (TM) {
+                tmem_fence16(dr[r]);
+                Regs6<T>::unpack(dr[r], del);
+                uint32_t pk[12];
+                Regs6<T>::pack(park[r], pk);
+                tmem_st8_nc(tdl + r * TBLOCK + n4 * DLCOLS, pk);
+                tmem_st4_nc(tdl + r * TBLOCK + n4 * DLCOLS + 8, pk + 8);
             } else {
 #pragma unroll
-                for (int q = 0; q < 6; ++q) del[q] = st[r].dl[q][r4];
-            }
-            const T(&win)[4][8] = st[r].win;
-#pragma unroll
-            for (int f = 0; f < 4; ++f) {
-                const T* a = f == 0 ? c.ar : c.au;
-                fc[f] = win[f][cz];
-                d1z[f] = fma_(a[2], win[f][(cz + 3) & 7] - win[f][(cz + 5) & 7],
-                              fma_(a[1], win[f][(cz + 2) & 7] - win[f][(cz + 6) & 7], a[0] * (win[f][(cz + 1) & 7] - win[f][(cz + 7) & 7])));
-            }
-            T lz[3];
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                const T* bz = i == 2 ? c.lq : c.lo;
-                const int f = i + 1;
-                T v = fma_(bz[0], fc[f], st[r].lin[i][cz]);
-                v = fma_(bz[1], win[f][(cz + 1) & 7] + win[f][(cz + 7) & 7], v);
-                v = fma_(bz[2], win[f][(cz + 2) & 7] + win[f][(cz + 6) & 7], v);
-                v = fma_(bz[3], win[f][(cz + 3) & 7] + win[f][(cz + 5) & 7], v);
-                lz[i] = v;
+                for (int q = 0; q < 6; ++q) {
+                    del[q] = st[r].dl[q][n4];
+                    st[r].dl[q][n4] = park[r][q];
+                }
             }
             const T gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
-            const T gz = d1z[0], Gxz = d1z[1], Gyz = d1z[2], Gzz = d1z[3], uz = fc[3];
+            const T gz = d1z[r][0], Gxz = d1z[r][1], Gyz = d1z[r][2], Gzz = d1z[r][3], uz = fc[r][3];
             const T divp = Dhd + Gzz;  // dt * div u
             T Rv[4];
             Rv[0] = fma_(-(c.dt * uz), gz, P0d - Gzz);
             const T ngz = c.nu * gz, m23 = c.nu23 * Gzz;
-            T rx = lz[0], ry = lz[1], rz = lz[2];
+            T rx = lz[r][0], ry = lz[r][1], rz = lz[r][2];
             rx = fma_(-uz, Gxz, rx);
             ry = fma_(-uz, Gyz, ry);
             rz = fma_(-uz, Gzz, rz);
@@ -432,13 +505,19 @@ struct Tiled {
             if constexpr (FORCE) {  // + dt f_i = dt N f_k,i cos(k.x + phi), cos(a + b) = cos a cos b - sin a sin b
                 T cxy = T(0), sxy = T(0);
                 if constexpr (TM) {
-                    if constexpr (FXY_LATE) {
-                        tmem_ld<4>(tdl + r * TBLOCK + FXYCOL, fr);
-                        tmem_wait_ld();
+                    if (n4 == 0) {  // the forcing's xy phase factors sit in the spare columns 12..15 of delay-line slot 0
+                        const uint2 uc = make_uint2(dr[r][12], dr[r][13]), us = make_uint2(dr[r][14], dr[r][15]);
+                        cxy = *reinterpret_cast<const T*>(&uc);
+                        sxy = *reinterpret_cast<const T*>(&us);
+                    } else {
+                        uint32_t fr[4];
+                        tmem_ld4_nc(tdl + r * TBLOCK + FXYCOL, fr);
+                        tmem_wait_ld_nc();
+                        tmem_fence4(fr);
+                        const uint2 uc = make_uint2(fr[0], fr[1]), us = make_uint2(fr[2], fr[3]);
+                        cxy = *reinterpret_cast<const T*>(&uc);
+                        sxy = *reinterpret_cast<const T*>(&us);
                     }
-                    const uint2 uc = make_uint2(fr[0], fr[1]), us = make_uint2(fr[2], fr[3]);
-                    cxy = *reinterpret_cast<const T*>(&uc);
-                    sxy = *reinterpret_cast<const T*>(&us);
                 } else if (ok[r]) {
                     ft.xy(ci, cj + r, cxy, sxy);  // L1-resident tables: no registers held across planes
                 }
@@ -447,12 +526,13 @@ struct Tiled {
                 for (int i = 0; i < 3; ++i) Rv[1 + i] = fma_(c.fa[i], cth, Rv[1 + i]);
             }
             // ---- Eq. 10; coalesced row segments per warp straight to global memory
-            if (ok[r]) {
+            if (ok[r] && out) {
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
-                    const T wn = c.read_w ? fma_(c.alpha, wsp[f * WFIELD + r * TX], Rv[f]) : Rv[f];
-                    if (c.write_w) bW[ow + f * n + r * pw] = wn;
-                    if (c.write_f) bF[of + f * fs + r * pf] = fma_(c.beta, wn, fc[f]);
+                    const T wold = wsp[f * WFIELD + r * TX];
+                    const T wn = RW ? fma_(c.alpha, wold, Rv[f]) : Rv[f];
+                    if (WW) bW[ow + f * n + r * pw] = wn;
+                    if (WF) bF[of + f * fs + r * pf] = fma_(c.beta, wn, fc[r][f]);
                 }
                 if (!PATH55) bD[of + r * pf] = divp;
             }
@@ -466,7 +546,7 @@ struct Tiled {
         T* smw = sm + NS * STAGE;
         const uint32_t a_sm = __reduce_or_sync(0xffffffffu, smem_u32(smem_raw));  // uniform: kept in a uniform register
         const uint32_t a_smw = a_sm + (uint32_t)(NS * STAGE * sizeof(T));
-        const uint32_t a_full = a_smw + (uint32_t)(NW * WSTAGE * sizeof(T)), a_empty = a_full + 8 * NS, a_wfull = a_empty + 8 * NS;
+        const uint32_t a_full = a_smw + (uint32_t)(NW * WSTAGE * sizeof(T)), a_empty = a_full + 8 * NS;
         const int tx = threadIdx.x, ty = threadIdx.y;
         const int tid = ty * TX + tx;
         const bool lane0 = (tid & 31) == 0, producer = tid == 0;
@@ -491,13 +571,11 @@ struct Tiled {
                 mbar_init(a_full + 8 * i, 1);
                 mbar_init(a_empty + 8 * i, WARPS);
             }
-#pragma unroll
-            for (int i = 0; i < NW; ++i) mbar_init(a_wfull + 8 * i, 1);
             asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         }
-        const uint32_t a_tmem = a_wfull + 8 * NW;  // shared word that receives the TMEM base address
+        const uint32_t a_tmem = a_empty + 8 * NS;  // shared word that receives the TMEM base address
         // FORCE: (cos, sin) of k_z z for the output planes of this item, behind the barriers
-        T* ftz = reinterpret_cast<T*>(smem_raw + (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + NW + 2) * sizeof(uint64_t));
+        T* ftz = reinterpret_cast<T*>(smem_raw + (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + 2) * sizeof(uint64_t));
         if constexpr (FORCE) {
             for (int i = tid; i < ze - zs; i += THREADS) ft.z(zs + i, ftz[2 * i], ftz[2 * i + 1]);
         }
@@ -564,56 +642,56 @@ struct Tiled {
                 for (int a = 0; a < 4; ++a) st[r].dl[q][a] = T(0);
         }
 
-        for (int pb = 0; pb < np; pb += 8) {
+        // Software-pipelined plane loop: iteration p stages nothing itself; it consumes plane p in-plane (p < np) and
+        // finishes output index p - 7 (p >= 7), both in plane<>().  np + 1 iterations; the last one has no new plane
+        // (its in-plane part re-reads a stale stage and only feeds ring slots that are never output).
+        const int niter = np + 1;
+        for (int pb = 0; pb < niter; pb += 8) {
 #pragma unroll
             for (int ph = 0; ph < 8; ++ph) {
                 const int p = pb + ph;
-                if (p < np) {
-                    const bool out = p >= 2 * R;  // planes 0..5 of a chunk only warm the window and the rings up
-                    if constexpr (TM) tmem_wait_st();  // what the previous planes parked in tensor memory is in place
-                    mbar_wait(a_full + 8 * (ph & (NS - 1)), (uint32_t)((p >> LNS) & 1));
-                    if (out && c.read_w) mbar_wait(a_wfull + 8 * ((ph + 2) & 3), (uint32_t)(((p - 2 * R) >> 2) & 1));
-#define FD6_STEP(K) \
-    step<K>(st, sp0, wsp0, tdl, c, out, Fout, W, Div, of, ow, (uint32_t)g.fs, (uint32_t)g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R))
+                if (p < niter) {
+                    const bool out = p >= 2 * R + 1;
+                    if constexpr (TM) tmem_wait_st_nc();  // what the previous iterations parked in tensor memory is in place
+                    // ONE barrier per iteration: plane p of F and the w values of output index p - 7 were requested together
+                    if (p < np || (RW && out)) mbar_wait(a_full + 8 * (ph & 3), (uint32_t)((p >> 2) & 1));
+#define FD6_PLANE(K) \
+    plane<K>(st, sp0, wsp0, tdl, c, out, Fout, W, Div, of, ow, (uint32_t)g.fs, (uint32_t)g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R - 1))
                     switch (ph) {  // ph is a compile-time constant after unrolling
-                        case 0: FD6_STEP(0); break;
-                        case 1: FD6_STEP(1); break;
-                        case 2: FD6_STEP(2); break;
-                        case 3: FD6_STEP(3); break;
-                        case 4: FD6_STEP(4); break;
-                        case 5: FD6_STEP(5); break;
-                        case 6: FD6_STEP(6); break;
-                        default: FD6_STEP(7); break;
+                        case 0: FD6_PLANE(0); break;
+                        case 1: FD6_PLANE(1); break;
+                        case 2: FD6_PLANE(2); break;
+                        case 3: FD6_PLANE(3); break;
+                        case 4: FD6_PLANE(4); break;
+                        case 5: FD6_PLANE(5); break;
+                        case 6: FD6_PLANE(6); break;
+                        default: FD6_PLANE(7); break;
                     }
+#undef FD6_PLANE
                     if (out && store_ok) {
                         ow += plane_w;
                         of += plane_f;
                     }
                     // this warp is done reading stage ph (F) and its w slot: hand them back
                     __syncwarp();
-                    if (lane0) mbar_arrive(a_empty + 8 * (ph & (NS - 1)));
-                    // thread 0 refills the stage every warp has released one plane earlier, so it never waits for a
-                    // warp that is less than a plane behind; the w values of step q = p + 3 go into the slot step p - 1 used
+                    if (lane0) mbar_arrive(a_empty + 8 * (ph & 3));
+                    // thread 0 requests what iteration q = p + 3 will consume into the stage and w slot that every warp has
+                    // released one iteration earlier: plane q of F and the w values of output index q - 7, on one barrier
                     if (producer && p >= 1) {
-                        const int sprev = (ph + 7) & (NS - 1);
-                        const bool more_f = p - 1 + NS < np;
+                        const int sq = (ph + 3) & 3;  // stage of iterations p - 1 and p + 3
                         const int q = p + 3;
-                        const bool more_w = c.read_w && q >= 2 * R && q < np;
-                        if (more_f || more_w) mbar_wait(a_empty + 8 * sprev, (uint32_t)(((p - 1) >> LNS) & 1));
-                        if (more_f) {
-                            mbar_expect_tx(a_full + 8 * sprev, kStageBytes);
-                            tma_load_4d(a_sm + sprev * kStageBytes, &m.f_in, a_full + 8 * sprev, bx, by, bz + p - 1 + NS, 0);
-                        }
-                        if (more_w) {
-                            const int ws = (ph + 5) & 3;  // (q - 6) & 3
-                            mbar_expect_tx(a_wfull + 8 * ws, kWBytes);
-                            tma_load_4d(a_smw + ws * kWBytes, &m.w_ld, a_wfull + 8 * ws, X0 * L, Y0, zs + q - 2 * R, 0);
+                        const bool more_f = q < np;
+                        const bool more_w = RW && q >= 2 * R + 1 && q < niter;
+                        if (more_f || more_w) {
+                            mbar_wait(a_empty + 8 * sq, (uint32_t)(((p - 1) >> 2) & 1));
+                            mbar_expect_tx(a_full + 8 * sq, (more_f ? kStageBytes : 0u) + (more_w ? kWBytes : 0u));
+                            if (more_f) tma_load_4d(a_sm + sq * kStageBytes, &m.f_in, a_full + 8 * sq, bx, by, bz + q, 0);
+                            if (more_w) tma_load_4d(a_smw + (ph & 3) * kWBytes, &m.w_ld, a_full + 8 * sq, X0 * L, Y0, zs + q - 2 * R - 1, 0);
                         }
                     }
                 }
             }
         }
-#undef FD6_STEP
         if constexpr (TM) {
             asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
             __syncthreads();
@@ -622,11 +700,11 @@ struct Tiled {
     }
 };
 
-template <class T, bool PATH55, int TX, int TY, int NS, int RY, bool FORCE>
+template <class T, bool PATH55, int TX, int TY, int NS, int RY, bool FORCE, int MODE>
 __global__ void __launch_bounds__(TX* TY, 1)
     k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, const Sched sc, T* __restrict__ Fout,
                  T* __restrict__ W, T* __restrict__ Div, const ForceTab<T> ft) {
-    Tiled<T, PATH55, TX, TY, NS, RY, FORCE>::run(m, g, c, sc, Fout, W, Div, ft);
+    Tiled<T, PATH55, TX, TY, NS, RY, FORCE, MODE>::run(m, g, c, sc, Fout, W, Div, ft);
 }
 
 // Tile shape per value type (registers per thread bound the CTA size).  RY = 2 (two vertically
@@ -642,9 +720,15 @@ template <>
 struct TileShape<double> {
     static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x 168 registers: window and delay line in tensor memory
 };
+#ifndef FD6_V2_TY
+#define FD6_V2_TY 12
+#endif
+#ifndef FD6_V2_RY
+#define FD6_V2_RY 1
+#endif
 template <>
 struct TileShape<V2> {
-    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x <= 168 registers: window and delay line in tensor memory
+    static constexpr int TX = 32, TY = FD6_V2_TY, NS = 4, RY = FD6_V2_RY;  // 12 warps x <= 168 registers: window and delay line in tensor memory
 };
 
 // ---- host side -------------------------------------------------------------------------------------------
@@ -733,6 +817,30 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     return sc;
 }
 
+// Every instantiation of the main kernel for value type T: fn(kernel, force, path55, mode) (or fn(kernel, force)).
+template <class T, bool P55, bool FORCE, int MODE, class Fn>
+static void each_kernel_1(Fn&& fn) {
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
+    if constexpr (std::is_invocable_v<Fn, decltype(&k_tiled_main<T, P55, TX, TY, NS, RY, FORCE, MODE>), bool>)
+        fn(&k_tiled_main<T, P55, TX, TY, NS, RY, FORCE, MODE>, FORCE);
+    else
+        fn(&k_tiled_main<T, P55, TX, TY, NS, RY, FORCE, MODE>, FORCE, P55, MODE);
+}
+template <class T, bool P55, bool FORCE, class Fn>
+static void each_kernel_2(Fn&& fn) {
+    each_kernel_1<T, P55, FORCE, 6>(fn);  // substep 1
+    each_kernel_1<T, P55, FORCE, 7>(fn);  // substep 2
+    each_kernel_1<T, P55, FORCE, 5>(fn);  // substep 3
+    each_kernel_1<T, P55, FORCE, 2>(fn);  // fd_rhs
+}
+template <class T, class Fn>
+static void for_each_kernel(Fn&& fn) {
+    each_kernel_2<T, true, false>(fn);
+    each_kernel_2<T, false, false>(fn);
+    each_kernel_2<T, true, true>(fn);
+    each_kernel_2<T, false, true>(fn);
+}
+
 // F[0], F[1]: the two padded copies; W: the dense w arrays.
 template <class T>
 static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
@@ -746,15 +854,14 @@ static int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
         if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY * RY, 4);
     }
     if (rc) return rc;
-    const int smem = (int)Tiled<T, true, TX, TY, NS, RY, false>::SMEM;  // the same for all four instantiations
-    cudaError_t e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    const int smem_f = (int)Tiled<T, true, TX, TY, NS, RY, true>::smem_bytes(g.nz);  // + the forcing's z table
+    const int smem = (int)Tiled<T, true, TX, TY, NS, RY, false, 7>::SMEM;  // the same for every instantiation
+    const int smem_f = (int)Tiled<T, true, TX, TY, NS, RY, true, 7>::smem_bytes(g.nz);  // + the forcing's z table
     ts.force_fits = smem_f <= 227 * 1024;
-    if (ts.force_fits) {
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, true, TX, TY, NS, RY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_f);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(k_tiled_main<T, false, TX, TY, NS, RY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_f);
-    }
+    cudaError_t e = cudaSuccess;
+    for_each_kernel<T>([&](auto kernel, bool force) {
+        if (e == cudaSuccess && (!force || ts.force_fits))
+            e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, force ? smem_f : smem);
+    });
     if (e != cudaSuccess) {
         snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
         cudaGetLastError();
@@ -814,22 +921,26 @@ template <class T>
 static int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
                              const ForceTab<T>& ft, cudaStream_t stream) {
     constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
-    constexpr size_t SMEM = Tiled<T, true, TX, TY, NS, RY, false>::SMEM;
+    constexpr size_t SMEM = Tiled<T, true, TX, TY, NS, RY, false, 7>::SMEM;
     dim3 block(TX, TY, 1), grid(ts.items, 1, 1);
-    if (ft.tab == nullptr) {
-        if (path55)
-            k_tiled_main<T, true, TX, TY, NS, RY, false><<<grid, block, SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
-        else
-            k_tiled_main<T, false, TX, TY, NS, RY, false><<<grid, block, SMEM, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
-    } else {
-        if (!ts.force_fits) return 4;
-        const size_t smem_f = Tiled<T, true, TX, TY, NS, RY, true>::smem_bytes(g.nz);
-        if (path55)
-            k_tiled_main<T, true, TX, TY, NS, RY, true><<<grid, block, smem_f, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
-        else
-            k_tiled_main<T, false, TX, TY, NS, RY, true><<<grid, block, smem_f, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+    const bool force = ft.tab != nullptr;
+    if (force && !ts.force_fits) return 4;
+    const size_t smem = force ? Tiled<T, true, TX, TY, NS, RY, true, 7>::smem_bytes(g.nz) : SMEM;
+    const int mode = (c.read_w ? 1 : 0) | (c.write_w ? 2 : 0) | (c.write_f ? 4 : 0);
+    bool launched = false;
+    for_each_kernel<T>([&](auto kernel, bool kforce, bool k55, int kmode) {
+        if (!launched && kforce == force && k55 == (path55 != 0) && kmode == mode) {
+            kernel<<<grid, block, smem, stream>>>(ts.maps[cur], g, c, ts.sched, Fout, W, Div, ft);
+            launched = true;
+        }
+    });
+    if (!launched) {
+        snprintf(ts.err, sizeof(ts.err), "no tiled kernel for update mode %d", mode);
+        return 3;
     }
-    return cudaGetLastError() == cudaSuccess ? 0 : 3;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) snprintf(ts.err, sizeof(ts.err), "%s", cudaGetErrorString(e));
+    return e == cudaSuccess ? 0 : 3;
 }
 
 }  // namespace fd6
