@@ -13,7 +13,7 @@
 
 #include "fd6_common.cuh"
 #include "fd6_kernels_direct.cuh"
-#include "fd6_kernels_tiled.cuh"
+#include "fd6_tiled_host.cuh"
 
 using namespace fd6;
 

@@ -1,0 +1,263 @@
+// fd6_tiled_host.cuh — host side of FD_VARIANT_TILED / FD_VARIANT_PAIRED: launch parameters, tile shapes, tensor maps,
+// the work-list planner and the launch wrappers.  The kernels themselves are in fd6_kernels_tiled.cuh and are compiled
+// in translation units of their own (fd6_tiled_inst.cu); fd6.cu sees only this file.
+#pragma once
+#include <cuda.h>
+
+#include <cstdio>
+
+#include "fd6_common.cuh"
+
+namespace fd6 {
+
+// Coefficients with the physics constants, dt and the RK substep folded in (formed in double on the host,
+// rounded once to the scalar type; V2 holds the same number in both halves).
+template <class T>
+struct KC {
+    T ar[3];   // Eq. 6:  a_m / (60 dx)                     first derivatives of ln rho
+    T au[3];   // dt a_m / (60 dx)                          first derivatives of u (carry dt)
+    T lo[4];   // dt nu b_m / (180 dx^2), m = 0..3          second derivative along an axis other than i
+    T lq[4];   // PATH55: dt (4 nu / 3) b_m (d_ii u_i enters lap u_i and d_i div u);  PATH19: same as lo
+    T cxy[3];  // centre coefficient of the in-plane second derivatives of u_x, u_y, u_z
+    T mq[3];   // dt (nu / 3) c_m / (720 dx^2)              Eq. 8
+    T nu, nu2, nu23, cs2dt, dt;
+    T alpha, beta;
+    T fa[3];   // FORCE: dt N f_k (Eq. 24-25), the amplitude of the forcing term in dt*rhs_i
+    int read_w, write_f, write_w;
+};
+
+// Work list of one launch (1-D grid, one CTA per item, launched in this order).  The first n_full tiles (a
+// multiple of the SM count) are marched through all of z by one CTA each; the remaining tiles, which would
+// fill only part of a last wave, are cut into k z-chunks of zc planes so that their items fill whole waves
+// again (each chunk re-stages 6 warm-up planes, which is why only the remainder is cut).
+struct Sched {
+    int ntx;     // tiles along x; tile index = bx + ntx * by
+    int n_full;  // tiles with a single item
+    int k, zc;   // chunks per remaining tile, planes per chunk
+};
+
+// The tensor maps of one launch (each 128 bytes, passed by value as a __grid_constant__ parameter).
+struct Maps {
+    CUtensorMap f_in;  // padded fields, read copy: box (TX+8, TY+6, 1, 4)
+    CUtensorMap w_ld;  // dense w:                  box (TX, TY, 1, 4)
+};
+
+// Tile shape per value type (registers per thread bound the CTA size).  RY = 2 (two vertically
+// adjacent outputs per thread, 13 % fewer shared-memory loads per value, 217 registers, 8 warps) is bit-identical
+// and was measured 1.5 % slower than RY = 1 with 12 warps for the paired fused kernel, 2 % faster for pass 1.
+template <class T>
+struct TileShape;
+template <>
+struct TileShape<float> {
+    static constexpr int TX = 64, TY = 8, NS = 4, RY = 1;  // 16 warps x 128 registers, state in registers (4 stages: 4 % faster than 8)
+};
+template <>
+struct TileShape<double> {
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x 168 registers: window and delay line in tensor memory
+};
+#ifndef FD6_V2_TY
+#define FD6_V2_TY 12
+#endif
+#ifndef FD6_V2_RY
+#define FD6_V2_RY 1
+#endif
+template <>
+struct TileShape<V2> {
+    static constexpr int TX = 32, TY = FD6_V2_TY, NS = 4, RY = FD6_V2_RY;  // 12 warps x <= 168 registers: window and delay line in tensor memory
+};
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                    CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct TiledState {
+    bool ready = false;
+    Maps maps[2];      // maps[cur]: read copy F[cur]
+    bool force_fits = true;  // the forcing's z table fits in shared memory beside the rings
+    Sched sched{};     // work list
+    int items = 0;     // grid size
+    int sm_count = 0;
+    char err[256] = "";
+};
+
+inline bool tiled_supported(const Geom& g) {  // the kernels address F_out and w with 32-bit element offsets
+    return g.nx >= 4 && g.ny >= 4 && g.nz >= 4 && 4 * g.fs < (1LL << 32) && 4 * g.n < (1LL << 32);
+}
+
+inline PFN_encodeTiled tiled_encode_fn() {
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (PFN_encodeTiled)p;
+        else
+            cudaGetLastError();
+    }
+    return fn;
+}
+
+// 4-D tensor map over `nf` arrays of (ex, ey, ez) values with pitches (px, py) and array stride fs (all in
+// values); the x extent and the box are given in values and converted to scalars here.
+template <class T>
+inline int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, long long ex, long long ey, long long ez, int nf, long long px,
+                          long long py, long long fs, int box_x, int box_y, int box_f) {
+    typedef typename Scalar<T>::type S;
+    constexpr int L = Scalar<T>::lanes;
+    PFN_encodeTiled enc = tiled_encode_fn();
+    if (!enc) {
+        snprintf(ts.err, sizeof(ts.err), "cuTensorMapEncodeTiled is not available from this driver");
+        return 3;
+    }
+    const cuuint64_t dims[4] = {(cuuint64_t)ex * L, (cuuint64_t)ey, (cuuint64_t)ez, (cuuint64_t)nf};
+    const cuuint64_t strides[3] = {(cuuint64_t)px * sizeof(T), (cuuint64_t)px * py * sizeof(T), (cuuint64_t)fs * sizeof(T)};
+    const cuuint32_t box[4] = {(cuuint32_t)(box_x * L), (cuuint32_t)box_y, 1, (cuuint32_t)box_f};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    CUresult r = enc(tm, sizeof(S) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 4, base, dims, strides, box,
+                     estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                     CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(ts.err, sizeof(ts.err), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+        return 3;
+    }
+    return 0;
+}
+
+// Work list (see Sched; pure host arithmetic, also reachable through fd_plan_work_list for the CPU tests): one CTA
+// per SM is resident, so whole waves of S tiles run as full columns and the remaining tiles are cut into the
+// number of z-chunks that minimises (waves x planes staged per item).
+inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
+    const int tiles = ntx * nty;
+    const int n_full = (tiles / S) * S, rem = tiles - n_full;
+    int best_k = 1;
+    double best_cost = 1e300;
+    for (int k = 1; rem > 0 && k <= (nz + 7) / 8 && k <= 64; ++k) {
+        const int zc = (nz + k - 1) / k;
+        const int real = (nz + zc - 1) / zc;
+        const long long waves = ((long long)rem * real + S - 1) / S;
+        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per item (+ fill latency)
+        if (cost < best_cost) {
+            best_cost = cost;
+            best_k = k;
+        }
+    }
+    Sched sc;
+    sc.ntx = ntx;
+    sc.n_full = n_full;
+    sc.zc = (nz + best_k - 1) / best_k;
+    sc.k = (nz + sc.zc - 1) / sc.zc;
+    *items = n_full + rem * sc.k;
+    return sc;
+}
+
+// The kernel instantiations of one value type live in translation units of their own (fd6_tiled_inst.cu, one per
+// value type and FORCE; compiled in parallel by build.py): this is the whole interface between them and fd6.cu.
+template <class T, bool FORCE>
+struct TiledTU {
+    static size_t smem_bytes(int planes);                 // dynamic shared memory of a launch over `planes` stored planes
+    static cudaError_t set_smem(size_t bytes);            // opt every instantiation of this unit in to `bytes`
+    static int max_ctas_per_sm(size_t bytes);             // occupancy of the fused kernel (the design assumes 1)
+    // launches the instantiation for (path55, mode); false if there is none
+    static bool launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g, const KC<T>& c,
+                       const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft);
+};
+
+// F[0], F[1]: the two padded copies; W: the dense w arrays.
+template <class T>
+inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
+    ts.ready = false;
+    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, RY = TileShape<T>::RY;
+    void* F[2] = {F0, F1};
+    int rc = 0;
+    for (int cur = 0; cur < 2 && rc == 0; ++cur) {
+        Maps& m = ts.maps[cur];
+        rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TY * RY + 2 * R, 4);
+        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY * RY, 4);
+    }
+    if (rc) return rc;
+    const size_t smem = TiledTU<T, false>::smem_bytes(0);
+    const size_t smem_f = TiledTU<T, true>::smem_bytes(g.nz);  // + the forcing's z table
+    ts.force_fits = smem_f <= 227 * 1024;
+    cudaError_t e = TiledTU<T, false>::set_smem(smem);
+    if (e == cudaSuccess && ts.force_fits) e = TiledTU<T, true>::set_smem(smem_f);
+    if (e != cudaSuccess) {
+        snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
+        cudaGetLastError();
+        return 3;
+    }
+    // the kernels take all of tensor memory and the work list counts waves of one CTA per SM
+    if (TiledTU<T, false>::max_ctas_per_sm(smem) != 1) {
+        snprintf(ts.err, sizeof(ts.err), "the tiled kernels are designed for exactly one resident CTA per SM");
+        return 3;
+    }
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (ts.sm_count <= 0) ts.sm_count = 148;
+    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TY * RY - 1) / (TY * RY), g.nz, ts.sm_count, &ts.items);
+    ts.ready = true;
+    return 0;
+}
+
+inline const char* tiled_error_of(const TiledState& ts) { return ts.err; }
+inline void tiled_release(TiledState& ts) { ts.ready = false; }
+
+template <class T>
+inline KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, double alpha, double beta, int read_w, int write_f,
+                     int write_w, const double famp[3]) {
+    typedef typename Scalar<T>::type S;
+    const double dx2 = dx * dx;
+    const double b[4] = {-490.0 / (180.0 * dx2), 270.0 / (180.0 * dx2), -27.0 / (180.0 * dx2), 2.0 / (180.0 * dx2)};
+    const double cm[3] = {270.0 / (720.0 * dx2), -27.0 / (720.0 * dx2), 2.0 / (720.0 * dx2)};
+    const double a[3] = {45.0 / (60.0 * dx), -9.0 / (60.0 * dx), 1.0 / (60.0 * dx)};
+    const double own = path55 ? 4.0 * nu / 3.0 : nu;
+    KC<T> k;
+    for (int m = 0; m < 3; ++m) {
+        k.ar[m] = T(S(a[m]));
+        k.au[m] = T(S(dt * a[m]));
+        k.mq[m] = T(S(dt * nu / 3.0 * cm[m]));
+    }
+    for (int m = 0; m < 4; ++m) {
+        k.lo[m] = T(S(dt * nu * b[m]));
+        k.lq[m] = T(S(dt * own * b[m]));
+    }
+    k.cxy[0] = T(S(dt * (own + nu) * b[0]));
+    k.cxy[1] = T(S(dt * (own + nu) * b[0]));
+    k.cxy[2] = T(S(dt * 2.0 * nu * b[0]));
+    k.nu = T(S(nu));
+    k.nu2 = T(S(2.0 * nu));
+    k.nu23 = T(S(2.0 * nu / 3.0));
+    k.cs2dt = T(S(cs * cs * dt));
+    k.dt = T(S(dt));
+    k.alpha = T(S(alpha));
+    k.beta = T(S(beta));
+    for (int i = 0; i < 3; ++i) k.fa[i] = T(S(dt * famp[i]));
+    k.read_w = read_w;
+    k.write_f = write_f;
+    k.write_w = write_w;
+    return k;
+}
+
+// Launch of the main kernel of one substep (fused 55-point kernel, or pass 1 of the 19-point path, which
+// leaves dt * div u in Div): reads copy `cur`, writes copy 1 - cur and w.
+template <class T>
+inline int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
+                             const ForceTab<T>& ft, cudaStream_t stream) {
+    const bool force = ft.tab != nullptr;
+    if (force && !ts.force_fits) return 4;
+    const int mode = (c.read_w ? 1 : 0) | (c.write_w ? 2 : 0) | (c.write_f ? 4 : 0);
+    const bool launched = force ? TiledTU<T, true>::launch(path55 != 0, mode, ts.items, TiledTU<T, true>::smem_bytes(g.nz), stream, ts.maps[cur],
+                                                           g, c, ts.sched, Fout, W, Div, ft)
+                                : TiledTU<T, false>::launch(path55 != 0, mode, ts.items, TiledTU<T, false>::smem_bytes(0), stream, ts.maps[cur],
+                                                            g, c, ts.sched, Fout, W, Div, ft);
+    if (!launched) {
+        snprintf(ts.err, sizeof(ts.err), "no tiled kernel for update mode %d", mode);
+        return 3;
+    }
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) snprintf(ts.err, sizeof(ts.err), "%s", cudaGetErrorString(e));
+    return e == cudaSuccess ? 0 : 3;
+}
+
+}  // namespace fd6
