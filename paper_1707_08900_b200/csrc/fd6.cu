@@ -282,7 +282,8 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
     {
         LaunchScope ls(c, p55 ? FD_K_FUSED55 : FD_K_PASS1);
         if (tiled) {
-            const KC<T> kc = make_kc<T>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w,
+            typedef typename Arith<T>::type A;  // the arithmetic type of the tiled kernels (V2 for plain fp32)
+            const KC<A> kc = make_kc<A>(c->dx, c->nu, c->cs, p55, sd.dt, sd.alpha, sd.beta, sd.read_w, sd.write_f, sd.write_w,
                                         c->force_on ? c->famp : no_force);
             const int lrc = tiled_launch_main<T>(c->tiled, p55, c->cur, Fout, W, Div, g, kc, ft, c->stream);
             if (lrc == 4) return fail(FD_EUNSUPPORTED, "forcing on a grid with this many planes needs FD_VARIANT_DIRECT");
@@ -783,13 +784,13 @@ extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count
     int tx, ty;
     if (dtype == FD_F64) {
         tx = TileShape<double>::TX;
-        ty = TileShape<double>::TY * TileShape<double>::RY;
+        ty = TileShape<double>::TH;
     } else if (paired) {
         tx = TileShape<V2>::TX;
-        ty = TileShape<V2>::TY * TileShape<V2>::RY;
+        ty = TileShape<V2>::TH;
     } else {
         tx = TileShape<float>::TX;
-        ty = TileShape<float>::TY * TileShape<float>::RY;
+        ty = TileShape<float>::TH;
     }
     const int planes = paired ? nz / 2 : nz;
     int items = 0;

@@ -203,8 +203,12 @@ struct Regs6 {
 // written), 2 = fd_rhs (w <- rhs only).
 template <class T, bool PATH55, int TX, int TY, int NS_, int RY, bool FORCE, int MODE>
 struct Tiled {
+    typedef typename Arith<T>::type A;  // arithmetic type: T itself, or V2 = two vertically adjacent fp32 cells (plain fp32)
+    static constexpr int CY = Arith<T>::CY;
+    static constexpr bool YP = CY == 2;   // "y pairs": T = float in memory, one thread computes cells (i, j) and (i, j+1) as one V2
+    static_assert(!YP || RY == 1, "y pairs: one value (two cells) per thread");
     static constexpr bool RW = (MODE & 1) != 0, WW = (MODE & 2) != 0, WF = (MODE & 4) != 0;
-    static constexpr int TH = TY * RY;  // tile height in values
+    static constexpr int TH = TY * RY * CY;  // tile height in stored elements (cells, or paired-layout values)
     static constexpr int PXS = TX + 8;  // staged row: 4 values left of the tile (3 used; keeps rows 16-byte aligned) + TX + 4
     static constexpr int PYS = TH + 2 * R;
     static constexpr int FIELD = PXS * PYS;
@@ -219,28 +223,28 @@ struct Tiled {
     // Tensor memory as per-thread storage (8-byte value types): a warp owns the 32 lanes of its quadrant (warp % 4);
     // the warps of a quadrant use different column blocks, one per owned column.  Block = 4 delay-line slots of 16
     // columns (6 values) + 4 fields x 8 window slots of 2 columns = 128 columns.  TMEM is otherwise idle here.
-    static constexpr bool TM = sizeof(T) == 8;
+    static constexpr bool TM = sizeof(A) == 8;
     static constexpr int DLCOLS = 16, TWIN = 4 * DLCOLS, TBLOCK = TWIN + 4 * 16;
     static constexpr int FXYCOL = 12;  // spare columns 12..15 of delay-line slot 0: the forcing's xy phase factors
     // when to fetch them: with the window (fp64) or after the right-hand side is assembled (paired fp32, where the
     // register pressure peaks at the window load: 144 registers and no spill instead of 168 with spills) — measured
-    static constexpr bool FXY_LATE = Scalar<T>::lanes == 2;
+    static constexpr bool FXY_LATE = Scalar<A>::lanes == 2;
     static constexpr int TMEM_NEED = ((WARPS + 3) / 4) * RY * TBLOCK;
     static constexpr int TMEM_COLS = TMEM_NEED <= 128 ? 128 : (TMEM_NEED <= 256 ? 256 : 512);
     static_assert(TMEM_NEED <= 512, "tensor memory has 512 columns");
     static constexpr size_t SMEM = (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + 2) * sizeof(uint64_t);
-    static size_t smem_bytes(int planes) { return SMEM + (FORCE ? 2 * (size_t)planes * sizeof(T) : 0); }  // + the z table
+    static size_t smem_bytes(int planes) { return SMEM + (FORCE ? 2 * (size_t)planes * sizeof(A) : 0); }  // + the z table
     static_assert((STAGE * sizeof(T)) % 128 == 0 && (WSTAGE * sizeof(T)) % 128 == 0, "TMA shared-memory boxes must stay 128-byte aligned");
 
     struct State {   // of one owned column
-        T win[4][8];
-        T lin[3][8];
-        T dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of the last planes (registers: !TM only)
+        A win[4][8];
+        A lin[3][8];
+        A dl[6][4];  // g_x, g_y, d_x u_z, d_y u_z, d_x u_x + d_y u_y, partial rhs_0 of the last planes (registers: !TM only)
     };
 
     // scatter of the in-plane differences e_m of plane t into the accumulator ring of one rhs component (Eq. 8 with z)
     template <int n8>
-    static __device__ __forceinline__ void scatter(T (&lin)[8], const T (&e)[3], const KC<T>& c) {
+    static __device__ __forceinline__ void scatter(A (&lin)[8], const A (&e)[3], const KC<A>& c) {
         lin[(n8 + 3) & 7] = (-c.mq[2]) * e[2];  // first contribution to output t+3 (the sign goes with the constant: free)
         lin[(n8 + 2) & 7] = fma_(-c.mq[1], e[1], lin[(n8 + 2) & 7]);
         lin[(n8 + 1) & 7] = fma_(-c.mq[0], e[0], lin[(n8 + 1) & 7]);
@@ -253,27 +257,27 @@ struct Tiled {
     // accumulator, from the window ring (slot t = n8 is not among the seven used).  wr: the ring of field f as fetched
     // from tensor memory (after tcgen05.wait::ld); plain fp32: the ring is st.win[f] and slot t is rewritten with cnew.
     template <int n8>
-    static __device__ __forceinline__ void zfield(int f, State& st, uint32_t (&wr)[16], T cnew, T (&fc)[4], T (&d1z)[4], T (&lz)[3], const KC<T>& c) {
+    static __device__ __forceinline__ void zfield(int f, State& st, uint32_t (&wr)[16], A cnew, A (&fc)[4], A (&d1z)[4], A (&lz)[3], const KC<A>& c) {
         constexpr int cz = (n8 + 4) & 7;
-        T w8[8];
+        A w8[8];
         if constexpr (TM) {
             tmem_fence16(wr);
 #pragma unroll
             for (int a8 = 0; a8 < 8; ++a8) {
                 const uint2 u = make_uint2(wr[2 * a8], wr[2 * a8 + 1]);
-                w8[a8] = *reinterpret_cast<const T*>(&u);
+                w8[a8] = *reinterpret_cast<const A*>(&u);
             }
         } else {
 #pragma unroll
             for (int a8 = 0; a8 < 8; ++a8) w8[a8] = st.win[f][a8];
             st.win[f][n8] = cnew;  // after the read: slot t is unused by this output
         }
-        const T* a = f == 0 ? c.ar : c.au;
+        const A* a = f == 0 ? c.ar : c.au;
         fc[f] = w8[cz];
         d1z[f] = fma_(a[2], w8[(cz + 3) & 7] - w8[(cz + 5) & 7], fma_(a[1], w8[(cz + 2) & 7] - w8[(cz + 6) & 7], a[0] * (w8[(cz + 1) & 7] - w8[(cz + 7) & 7])));
         if (f > 0) {
-            const T* bz = f == 3 ? c.lq : c.lo;
-            T v = fma_(bz[0], fc[f], st.lin[f - 1][cz]);
+            const A* bz = f == 3 ? c.lq : c.lo;
+            A v = fma_(bz[0], fc[f], st.lin[f - 1][cz]);
             v = fma_(bz[1], w8[(cz + 1) & 7] + w8[(cz + 7) & 7], v);
             v = fma_(bz[2], w8[(cz + 2) & 7] + w8[(cz + 6) & 7], v);
             v = fma_(bz[3], w8[(cz + 3) & 7] + w8[(cz + 5) & 7], v);
@@ -296,13 +300,13 @@ struct Tiled {
     static constexpr bool SPLIT = RY > 1;
     template <int PH>
     static __device__ __forceinline__ void plane(State (&st)[RY], const T* __restrict__ sp0, const T* __restrict__ wsp0, uint32_t tdl,
-                                                 const KC<T>& c, bool out, T* __restrict__ bF, T* __restrict__ bW, T* __restrict__ bD, uint32_t of, uint32_t ow,
-                                                 uint32_t fs, uint32_t n, int pf, int pw, const bool (&ok)[RY], const ForceTab<T>& ft, int ci, int cj, const T* __restrict__ ftz) {
+                                                 const KC<A>& c, bool out, T* __restrict__ bF, T* __restrict__ bW, T* __restrict__ bD, uint32_t of, uint32_t ow,
+                                                 uint32_t fs, uint32_t n, int pf, int pw, const bool (&ok)[RY], bool okb, const ForceTab<T>& ft, int ci, int cj, const A* __restrict__ ftz) {
         constexpr int n8 = PH & 7, n4 = PH & 3;
         const T* sp = sp0 + (PH & 3) * STAGE;
         const T* wsp = wsp0 + ((PH + 1) & 3) * WSTAGE;  // w ring slot of output index p - 7
-        T ctr[RY][4], d1x[RY][4], d1y[RY][4], inpl[RY][3], ezx[RY][3];
-        T fc[RY][4], d1z[RY][4], lz[RY][3];
+        A ctr[RY][4], d1x[RY][4], d1y[RY][4], inpl[RY][3], ezx[RY][3];
+        A fc[RY][4], d1z[RY][4], lz[RY][3];
         uint32_t wr[RY][16];
         if constexpr (TM && !SPLIT) {
 #pragma unroll
@@ -313,31 +317,56 @@ struct Tiled {
             // ---- plane t, field f: in-plane derivatives (Eq. 6-8).  The RY + 6 values of the thread's own x column are
             // loaded once per field and serve the y stencils of all its outputs.
             const T* q0 = sp + f * FIELD;
-            T yv[RY + 2 * R];
+            A yv[YP ? 1 : RY + 2 * R];
+            if constexpr (!YP) {
 #pragma unroll
-            for (int i = 0; i < RY + 2 * R; ++i) yv[i] = q0[(i - R) * PXS];
+                for (int i = 0; i < RY + 2 * R; ++i) yv[i] = q0[(i - R) * PXS];
+            }
 #pragma unroll
             for (int r = 0; r < RY; ++r) {
                 const T* q = q0 + r * PXS;
-                ctr[r][f] = yv[r + R];
+                A xp1, xm1, xp2, xm2, xp3, xm3, dy1, dy2, dy3, sy1, sy2, sy3;
+                if constexpr (YP) {
+                    // the thread's cells are (x, a) and (x, b = a + 1), q points at (x, a).  Eight values of the x column
+                    // serve both y stencils; each enters ONE packed operand (so it is loaded straight into its half of a
+                    // register pair), the odd offsets are formed half by half with scalar instructions.
+                    typename Scalar<A>::type cy[8];
+#pragma unroll
+                    for (int k = 0; k < 8; ++k) cy[k] = q[(k - R) * PXS];
+                    ctr[r][f] = A(cy[3], cy[4]);
+                    const A up(cy[5], cy[6]), lo(cy[1], cy[2]);  // rows a+2, b+2 and a-2, b-2
+                    dy2 = up - lo;
+                    dy1 = A(cy[4] - cy[2], cy[5] - cy[3]);
+                    dy3 = A(cy[6] - cy[0], cy[7] - cy[1]);
+                    if (f > 0) {
+                        sy2 = up + lo;
+                        sy1 = A(cy[4] + cy[2], cy[5] + cy[3]);
+                        sy3 = A(cy[6] + cy[0], cy[7] + cy[1]);
+                    }
+                    xp1 = A(q[1], q[PXS + 1]); xm1 = A(q[-1], q[PXS - 1]);
+                    xp2 = A(q[2], q[PXS + 2]); xm2 = A(q[-2], q[PXS - 2]);
+                    xp3 = A(q[3], q[PXS + 3]); xm3 = A(q[-3], q[PXS - 3]);
+                } else {
+                    ctr[r][f] = yv[r + R];
+                    xp1 = q[1]; xm1 = q[-1]; xp2 = q[2]; xm2 = q[-2]; xp3 = q[3]; xm3 = q[-3];
+                    const A yp1 = yv[r + R + 1], ym1 = yv[r + R - 1], yp2 = yv[r + R + 2], ym2 = yv[r + R - 2], yp3 = yv[r + R + 3], ym3 = yv[r + R - 3];
+                    dy1 = yp1 - ym1; dy2 = yp2 - ym2; dy3 = yp3 - ym3;
+                    if (f > 0) { sy1 = yp1 + ym1; sy2 = yp2 + ym2; sy3 = yp3 + ym3; }
+                }
                 if constexpr (TM) {
                     const uint2 u = *reinterpret_cast<const uint2*>(&ctr[r][f]);
                     const uint32_t r2[2] = {u.x, u.y};
                     tmem_st2_nc(tdl + r * TBLOCK + TWIN + f * 16 + n8 * 2, r2);
                 }
-                const T xp1 = q[1], xm1 = q[-1], xp2 = q[2], xm2 = q[-2], xp3 = q[3], xm3 = q[-3];
-                const T yp1 = yv[r + R + 1], ym1 = yv[r + R - 1], yp2 = yv[r + R + 2], ym2 = yv[r + R - 2], yp3 = yv[r + R + 3], ym3 = yv[r + R - 3];
-                const T dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
-                const T dy1 = yp1 - ym1, dy2 = yp2 - ym2, dy3 = yp3 - ym3;
-                const T* a = f == 0 ? c.ar : c.au;
+                const A dx1 = xp1 - xm1, dx2 = xp2 - xm2, dx3 = xp3 - xm3;
+                const A* a = f == 0 ? c.ar : c.au;
                 d1x[r][f] = fma_(a[2], dx3, fma_(a[1], dx2, a[0] * dx1));
                 d1y[r][f] = fma_(a[2], dy3, fma_(a[1], dy2, a[0] * dy1));
                 if (f > 0) {
-                    const T sx1 = xp1 + xm1, sx2 = xp2 + xm2, sx3 = xp3 + xm3;
-                    const T sy1 = yp1 + ym1, sy2 = yp2 + ym2, sy3 = yp3 + ym3;
-                    const T* bx = f == 1 ? c.lq : c.lo;  // d_xx u_x and d_yy u_y carry 4nu/3 on the 55-point path
-                    const T* by = f == 2 ? c.lq : c.lo;
-                    T v = c.cxy[f - 1] * ctr[r][f];
+                    const A sx1 = xp1 + xm1, sx2 = xp2 + xm2, sx3 = xp3 + xm3;
+                    const A* bx = f == 1 ? c.lq : c.lo;  // d_xx u_x and d_yy u_y carry 4nu/3 on the 55-point path
+                    const A* by = f == 2 ? c.lq : c.lo;
+                    A v = c.cxy[f - 1] * ctr[r][f];
                     v = fma_(bx[1], sx1, v);
                     v = fma_(by[1], sy1, v);
                     v = fma_(bx[2], sx2, v);
@@ -345,10 +374,22 @@ struct Tiled {
                     v = fma_(bx[3], sx3, v);
                     v = fma_(by[3], sy3, v);
                     if (PATH55 && (f == 1 || f == 2)) {  // Eq. 8 in the xy plane: d_xy u_x -> rhs_y, d_xy u_y -> rhs_x
-                        const T q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
-                        const T q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
-                        const T q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
-                        const T dq = fma_(c.mq[2], q3, fma_(c.mq[1], q2, c.mq[0] * q1));
+                        A q1, q2, q3;
+                        if constexpr (YP) {
+                            // q_m = dx_m f(row + m) - dx_m f(row - m) for rows a and b.  m = 1: rows a + 1 = b and b - 1 = a
+                            // are the thread's own (dx1 above), only rows a - 1 and b + 1 are loaded
+                            const auto e_lo = q[-PXS + 1] - q[-PXS - 1], e_hi = q[2 * PXS + 1] - q[2 * PXS - 1];
+                            q1 = A(dx1.v.y - e_lo, e_hi - dx1.v.x);
+                            q2 = (A(q[2 * PXS + 2], q[3 * PXS + 2]) - A(q[2 * PXS - 2], q[3 * PXS - 2])) -
+                                 (A(q[-2 * PXS + 2], q[-PXS + 2]) - A(q[-2 * PXS - 2], q[-PXS - 2]));
+                            q3 = (A(q[3 * PXS + 3], q[4 * PXS + 3]) - A(q[3 * PXS - 3], q[4 * PXS - 3])) -
+                                 (A(q[-3 * PXS + 3], q[-2 * PXS + 3]) - A(q[-3 * PXS - 3], q[-2 * PXS - 3]));
+                        } else {
+                            q1 = (q[PXS + 1] - q[PXS - 1]) + (q[-PXS - 1] - q[-PXS + 1]);
+                            q2 = (q[2 * PXS + 2] - q[2 * PXS - 2]) + (q[-2 * PXS - 2] - q[-2 * PXS + 2]);
+                            q3 = (q[3 * PXS + 3] - q[3 * PXS - 3]) + (q[-3 * PXS - 3] - q[-3 * PXS + 3]);
+                        }
+                        const A dq = fma_(c.mq[2], q3, fma_(c.mq[1], q2, c.mq[0] * q1));
                         if (f == 1) { inpl[r][0] = v; inpl[r][1] = dq; } else { inpl[r][1] += v; inpl[r][0] += dq; }
                     } else {
                         inpl[r][f - 1] = v;
@@ -357,11 +398,11 @@ struct Tiled {
                 if (PATH55) {  // the differences that feed Dzx u_x + Dzy u_y -> rhs_z, Dxz u_z -> rhs_x, Dyz u_z -> rhs_y
                     if (f == 1) { ezx[r][0] = dx1; ezx[r][1] = dx2; ezx[r][2] = dx3; }
                     if (f == 2) {
-                        const T ez[3] = {ezx[r][0] + dy1, ezx[r][1] + dy2, ezx[r][2] + dy3};
+                        const A ez[3] = {ezx[r][0] + dy1, ezx[r][1] + dy2, ezx[r][2] + dy3};
                         scatter<n8>(st[r].lin[2], ez, c);
                     }
                     if (f == 3) {
-                        const T ex[3] = {dx1, dx2, dx3}, ey[3] = {dy1, dy2, dy3};
+                        const A ex[3] = {dx1, dx2, dx3}, ey[3] = {dy1, dy2, dy3};
                         scatter<n8>(st[r].lin[0], ex, c);
                         scatter<n8>(st[r].lin[1], ey, c);
                     }
@@ -386,18 +427,18 @@ struct Tiled {
             for (int r = 0; r < RY; ++r) tmem_ld16_nc(tdl + r * TBLOCK + n4 * DLCOLS, dr[r]);  // 12 values + 4 spare columns
         }
         // ---- plane t: everything of dt*rhs that needs no z derivative (Eq. 1-3); G' = dt * grad u
-        T park[RY][6];
+        A park[RY][6];
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
-            const T gx = d1x[r][0], gy = d1y[r][0], ux = ctr[r][1], uy = ctr[r][2];
-            const T Gxx = d1x[r][1], Gxy = d1y[r][1], Gyx = d1x[r][2], Gyy = d1y[r][2], Gzx = d1x[r][3], Gzy = d1y[r][3];
-            const T Dh = Gxx + Gyy;
-            const T ug = fma_(uy, gy, ux * gx);
-            const T P0 = fma_(-c.dt, ug, -Dh);
-            const T h = fma_(-c.nu23, Dh, -c.cs2dt);
-            const T nsym = c.nu * (Gxy + Gyx);
-            const T kx = fma_(c.nu2, Gxx, h), ky = fma_(c.nu2, Gyy, h);
-            T tx = inpl[r][0], ty = inpl[r][1], tz = inpl[r][2];
+            const A gx = d1x[r][0], gy = d1y[r][0], ux = ctr[r][1], uy = ctr[r][2];
+            const A Gxx = d1x[r][1], Gxy = d1y[r][1], Gyx = d1x[r][2], Gyy = d1y[r][2], Gzx = d1x[r][3], Gzy = d1y[r][3];
+            const A Dh = Gxx + Gyy;
+            const A ug = fma_(uy, gy, ux * gx);
+            const A P0 = fma_(-c.dt, ug, -Dh);
+            const A h = fma_(-c.nu23, Dh, -c.cs2dt);
+            const A nsym = c.nu * (Gxy + Gyx);
+            const A kx = fma_(c.nu2, Gxx, h), ky = fma_(c.nu2, Gyy, h);
+            A tx = inpl[r][0], ty = inpl[r][1], tz = inpl[r][2];
             tx = fma_(-ux, Gxx, tx);
             ty = fma_(-ux, Gyx, ty);
             tx = fma_(-uy, Gxy, tx);
@@ -408,7 +449,7 @@ struct Tiled {
             ty = fma_(nsym, gx, ty);
             tz = fma_(Gzx, fma_(c.nu, gx, -ux), tz);
             tz = fma_(Gzy, fma_(c.nu, gy, -uy), tz);
-            const T pl[3] = {tx, ty, tz};
+            const A pl[3] = {tx, ty, tz};
 #pragma unroll
             for (int i = 0; i < 3; ++i) {
                 if (PATH55)
@@ -433,12 +474,12 @@ struct Tiled {
 #pragma unroll
                 for (int f = 0; f < 4; ++f) zfield<n8>(f, st[r], w4[f], ctr[r][f], fc[r], d1z[r], lz[r], c);
             }
-            T del[6];
+            A del[6];
             if constexpr (TM) {
                 tmem_fence16(dr[r]);
-                Regs6<T>::unpack(dr[r], del);
+                Regs6<A>::unpack(dr[r], del);
                 uint32_t pk[12];
-                Regs6<T>::pack(park[r], pk);
+                Regs6<A>::pack(park[r], pk);
                 tmem_st8_nc(tdl + r * TBLOCK + n4 * DLCOLS, pk);
                 tmem_st4_nc(tdl + r * TBLOCK + n4 * DLCOLS + 8, pk + 8);
             } else {
@@ -448,13 +489,13 @@ struct Tiled {
                     st[r].dl[q][n4] = park[r][q];
                 }
             }
-            const T gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
-            const T gz = d1z[r][0], Gxz = d1z[r][1], Gyz = d1z[r][2], Gzz = d1z[r][3], uz = fc[r][3];
-            const T divp = Dhd + Gzz;  // dt * div u
-            T Rv[4];
+            const A gxd = del[0], gyd = del[1], Gzxd = del[2], Gzyd = del[3], Dhd = del[4], P0d = del[5];
+            const A gz = d1z[r][0], Gxz = d1z[r][1], Gyz = d1z[r][2], Gzz = d1z[r][3], uz = fc[r][3];
+            const A divp = Dhd + Gzz;  // dt * div u
+            A Rv[4];
             Rv[0] = fma_(-(c.dt * uz), gz, P0d - Gzz);
-            const T ngz = c.nu * gz, m23 = c.nu23 * Gzz;
-            T rx = lz[r][0], ry = lz[r][1], rz = lz[r][2];
+            const A ngz = c.nu * gz, m23 = c.nu23 * Gzz;
+            A rx = lz[r][0], ry = lz[r][1], rz = lz[r][2];
             rx = fma_(-uz, Gxz, rx);
             ry = fma_(-uz, Gyz, ry);
             rz = fma_(-uz, Gzz, rz);
@@ -469,25 +510,25 @@ struct Tiled {
             Rv[2] = ry;
             Rv[3] = rz;
             if constexpr (FORCE) {  // + dt f_i = dt N f_k,i cos(k.x + phi), cos(a + b) = cos a cos b - sin a sin b
-                T cxy = T(0), sxy = T(0);
+                A cxy = A(0), sxy = A(0);
                 if constexpr (TM) {
                     if (n4 == 0) {  // the forcing's xy phase factors sit in the spare columns 12..15 of delay-line slot 0
                         const uint2 uc = make_uint2(dr[r][12], dr[r][13]), us = make_uint2(dr[r][14], dr[r][15]);
-                        cxy = *reinterpret_cast<const T*>(&uc);
-                        sxy = *reinterpret_cast<const T*>(&us);
+                        cxy = *reinterpret_cast<const A*>(&uc);
+                        sxy = *reinterpret_cast<const A*>(&us);
                     } else {
                         uint32_t fr[4];
                         tmem_ld4_nc(tdl + r * TBLOCK + FXYCOL, fr);
                         tmem_wait_ld_nc();
                         tmem_fence4(fr);
                         const uint2 uc = make_uint2(fr[0], fr[1]), us = make_uint2(fr[2], fr[3]);
-                        cxy = *reinterpret_cast<const T*>(&uc);
-                        sxy = *reinterpret_cast<const T*>(&us);
+                        cxy = *reinterpret_cast<const A*>(&uc);
+                        sxy = *reinterpret_cast<const A*>(&us);
                     }
                 } else if (ok[r]) {
-                    ft.xy(ci, cj + r, cxy, sxy);  // L1-resident tables: no registers held across planes
+                    if constexpr (!YP) ft.xy(ci, cj + r, cxy, sxy);  // L1-resident tables: no registers held across planes
                 }
-                const T cth = fma_(-sxy, ftz[1], cxy * ftz[0]);
+                const A cth = fma_(-sxy, ftz[1], cxy * ftz[0]);
 #pragma unroll
                 for (int i = 0; i < 3; ++i) Rv[1 + i] = fma_(c.fa[i], cth, Rv[1 + i]);
             }
@@ -495,17 +536,37 @@ struct Tiled {
             if (ok[r] && out) {
 #pragma unroll
                 for (int f = 0; f < 4; ++f) {
-                    const T wold = wsp[f * WFIELD + r * TX];
-                    const T wn = RW ? fma_(c.alpha, wold, Rv[f]) : Rv[f];
-                    if (WW) bW[ow + f * n + r * pw] = wn;
-                    if (WF) bF[of + f * fs + r * pf] = fma_(c.beta, wn, fc[r][f]);
+                    if constexpr (YP) {  // row a, and row b = a + 1 when it is inside the grid
+                        A wold = A(0);
+                        if (RW) wold = A(wsp[f * WFIELD], wsp[f * WFIELD + TX]);
+                        const A wn = RW ? fma_(c.alpha, wold, Rv[f]) : Rv[f];
+                        const A fn = fma_(c.beta, wn, fc[r][f]);
+                        if (WW) bW[ow + f * n] = wn.v.x;
+                        if (WF) bF[of + f * fs] = fn.v.x;
+                        if (okb) {
+                            if (WW) bW[ow + f * n + pw] = wn.v.y;
+                            if (WF) bF[of + f * fs + pf] = fn.v.y;
+                        }
+                    } else {
+                        const A wold = wsp[f * WFIELD + r * TX];
+                        const A wn = RW ? fma_(c.alpha, wold, Rv[f]) : Rv[f];
+                        if (WW) bW[ow + f * n + r * pw] = wn;
+                        if (WF) bF[of + f * fs + r * pf] = fma_(c.beta, wn, fc[r][f]);
+                    }
                 }
-                if (!PATH55) bD[of + r * pf] = divp;
+                if constexpr (!PATH55) {
+                    if constexpr (YP) {
+                        bD[of] = divp.v.x;
+                        if (okb) bD[of + pf] = divp.v.y;
+                    } else {
+                        bD[of + r * pf] = divp;
+                    }
+                }
             }
         }
     }
 
-    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<T>& c, const Sched sc, T* __restrict__ Fout,
+    static __device__ __forceinline__ void run(const Maps& m, const Geom& g, const KC<A>& c, const Sched sc, T* __restrict__ Fout,
                                                T* __restrict__ W, T* __restrict__ Div, const ForceTab<T>& ft) {
         extern __shared__ __align__(128) unsigned char smem_raw[];
         T* sm = reinterpret_cast<T*>(smem_raw);
@@ -541,9 +602,13 @@ struct Tiled {
         }
         const uint32_t a_tmem = a_empty + 8 * NS;  // shared word that receives the TMEM base address
         // FORCE: (cos, sin) of k_z z for the output planes of this item, behind the barriers
-        T* ftz = reinterpret_cast<T*>(smem_raw + (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + 2) * sizeof(uint64_t));
+        A* ftz = reinterpret_cast<A*>(smem_raw + (size_t)(NS * STAGE + NW * WSTAGE) * sizeof(T) + (2 * NS + 2) * sizeof(uint64_t));
         if constexpr (FORCE) {
-            for (int i = tid; i < ze - zs; i += THREADS) ft.z(zs + i, ftz[2 * i], ftz[2 * i + 1]);
+            for (int i = tid; i < ze - zs; i += THREADS) {
+                T cz, sz;
+                ft.z(zs + i, cz, sz);
+                if constexpr (YP) { ftz[2 * i] = A(cz, cz); ftz[2 * i + 1] = A(sz, sz); } else { ftz[2 * i] = cz; ftz[2 * i + 1] = sz; }
+            }
         }
         uint32_t tmem_base = 0;
         if constexpr (TM) {
@@ -569,19 +634,28 @@ struct Tiled {
                 tma_load_4d(a_sm + i * kStageBytes, &m.f_in, a_full + 8 * i, bx, by, bz + i, 0);
             }
         }
-        const T* sp0 = sm + (ty * RY + R) * PXS + (tx + 4);
-        const T* wsp0 = smw + ty * RY * TX + tx;
+        const T* sp0 = sm + (ty * RY * CY + R) * PXS + (tx + 4);
+        const T* wsp0 = smw + ty * RY * CY * TX + tx;
         // this thread's first cell of output plane zs in the dense (w) and padded (F, div) arrays; advanced plane by plane
-        const int ci = X0 + tx, cj = Y0 + ty * RY;
+        const int ci = X0 + tx, cj = Y0 + ty * RY * CY;
         bool ok[RY];
 #pragma unroll
         for (int r = 0; r < RY; ++r) ok[r] = ci < g.nx && cj + r < g.ny;
         const bool store_ok = ok[0];
+        const bool okb = YP && ci < g.nx && cj + 1 < g.ny;  // y pairs: the second cell of the thread is inside the grid
         if constexpr (FORCE && TM) {
 #pragma unroll
             for (int r = 0; r < RY; ++r) {
-                T cxy = T(0), sxy = T(0);
-                if (ok[r]) ft.xy(ci, cj + r, cxy, sxy);
+                A cxy = A(0), sxy = A(0);
+                if constexpr (YP) {
+                    T ca = 0, sa = 0, cb = 0, sb = 0;
+                    if (ok[r]) ft.xy(ci, cj, ca, sa);
+                    if (okb) ft.xy(ci, cj + 1, cb, sb);
+                    cxy = A(ca, cb);
+                    sxy = A(sa, sb);
+                } else {
+                    if (ok[r]) ft.xy(ci, cj + r, cxy, sxy);
+                }
                 const uint2 uc = *reinterpret_cast<const uint2*>(&cxy), us = *reinterpret_cast<const uint2*>(&sxy);
                 const uint32_t r4[4] = {uc.x, uc.y, us.x, us.y};
                 tmem_st<4>(tdl + r * TBLOCK + FXYCOL, r4);
@@ -598,20 +672,23 @@ struct Tiled {
 #pragma unroll
             for (int a = 0; a < 8; ++a) {
 #pragma unroll
-                for (int f = 0; f < 4; ++f) st[r].win[f][a] = T(0);
+                for (int f = 0; f < 4; ++f) st[r].win[f][a] = A(0);
 #pragma unroll
-                for (int q = 0; q < 3; ++q) st[r].lin[q][a] = T(0);
+                for (int q = 0; q < 3; ++q) st[r].lin[q][a] = A(0);
             }
 #pragma unroll
             for (int q = 0; q < 6; ++q)
 #pragma unroll
-                for (int a = 0; a < 4; ++a) st[r].dl[q][a] = T(0);
+                for (int a = 0; a < 4; ++a) st[r].dl[q][a] = A(0);
         }
 
         // Software-pipelined plane loop: iteration p stages nothing itself; it consumes plane p in-plane (p < np) and
         // finishes output index p - 7 (p >= 7), both in plane<>().  np + 1 iterations; the last one has no new plane
         // (its in-plane part re-reads a stale stage and only feeds ring slots that are never output).
         const int niter = np + 1;
+        const int wid = tid >> 5;
+        int pwarp = 0;  // the warp whose lane 0 requests the loads at the end of this iteration: round robin over the warps, so
+                        // that no warp carries the producer's instructions and its wait for the slowest warp every iteration
         for (int pb = 0; pb < niter; pb += 8) {
 #pragma unroll
             for (int ph = 0; ph < 8; ++ph) {
@@ -622,7 +699,7 @@ struct Tiled {
                     // ONE barrier per iteration: plane p of F and the w values of output index p - 7 were requested together
                     if (p < np || (RW && out)) mbar_wait(a_full + 8 * (ph & 3), (uint32_t)((p >> 2) & 1));
 #define FD6_PLANE(K) \
-    plane<K>(st, sp0, wsp0, tdl, c, out, Fout, W, Div, of, ow, (uint32_t)g.fs, (uint32_t)g.n, g.px, g.nx, ok, ft, ci, cj, ftz + 2 * (p - 2 * R - 1))
+    plane<K>(st, sp0, wsp0, tdl, c, out, Fout, W, Div, of, ow, (uint32_t)g.fs, (uint32_t)g.n, g.px, g.nx, ok, okb, ft, ci, cj, ftz + 2 * (p - 2 * R - 1))
                     switch (ph) {  // ph is a compile-time constant after unrolling
                         case 0: FD6_PLANE(0); break;
                         case 1: FD6_PLANE(1); break;
@@ -643,7 +720,13 @@ struct Tiled {
                     if (lane0) mbar_arrive(a_empty + 8 * (ph & 3));
                     // thread 0 requests what iteration q = p + 3 will consume into the stage and w slot that every warp has
                     // released one iteration earlier: plane q of F and the w values of output index q - 7, on one barrier
-                    if (producer && p >= 1) {
+#ifdef FD6_FIXED_PRODUCER
+                    const bool requests = producer;
+#else
+                    const bool requests = lane0 && wid == pwarp;
+                    pwarp = pwarp + 1 == WARPS ? 0 : pwarp + 1;
+#endif
+                    if (requests && p >= 1) {
                         const int sq = (ph + 3) & 3;  // stage of iterations p - 1 and p + 3
                         const int q = p + 3;
                         const bool more_f = q < np;
@@ -668,7 +751,7 @@ struct Tiled {
 
 template <class T, bool PATH55, int TX, int TY, int NS, int RY, bool FORCE, int MODE>
 __global__ void __launch_bounds__(TX* TY, 1)
-    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<T> c, const Sched sc, T* __restrict__ Fout,
+    k_tiled_main(const __grid_constant__ Maps m, const Geom g, const __grid_constant__ KC<typename Arith<T>::type> c, const Sched sc, T* __restrict__ Fout,
                  T* __restrict__ W, T* __restrict__ Div, const ForceTab<T> ft) {
     Tiled<T, PATH55, TX, TY, NS, RY, FORCE, MODE>::run(m, g, c, sc, Fout, W, Div, ft);
 }
@@ -716,7 +799,8 @@ int TiledTU<T, FORCE>::max_ctas_per_sm(size_t bytes) {
     return n;
 }
 template <class T, bool FORCE>
-bool TiledTU<T, FORCE>::launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g, const KC<T>& c,
+bool TiledTU<T, FORCE>::launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g,
+                               const KC<typename Arith<T>::type>& c,
                                const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft) {
     dim3 block(TileShape<T>::TX, TileShape<T>::TY, 1), grid(items, 1, 1);
     bool launched = false;

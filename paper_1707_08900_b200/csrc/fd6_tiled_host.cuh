@@ -42,18 +42,26 @@ struct Maps {
     CUtensorMap w_ld;  // dense w:                  box (TX, TY, 1, 4)
 };
 
-// Tile shape per value type (registers per thread bound the CTA size).  RY = 2 (two vertically
-// adjacent outputs per thread, 13 % fewer shared-memory loads per value, 217 registers, 8 warps) is bit-identical
-// and was measured 1.5 % slower than RY = 1 with 12 warps for the paired fused kernel, 2 % faster for pass 1.
+// Arithmetic type of the kernels of storage type T.  fp64 and the paired layout compute on their stored value; PLAIN
+// fp32 computes on V2 = the two cells (i, j, k), (i, j+1, k) of one thread ("y pairs"): the pair shares the eight
+// values of its x column and its own-row x differences, every shared-memory access is a conflict-free 4-byte load
+// with consecutive lanes on consecutive words, and all arithmetic except the odd y offsets is packed (FFMA2).
+template <class T> struct Arith { typedef T type; static constexpr int CY = 1; };
+template <> struct Arith<float> { typedef V2 type; static constexpr int CY = 2; };
+
+// Tile shape per value type (registers per thread bound the CTA size).  TX x TY threads; a thread
+// owns RY columns of values, a value of the arithmetic type holds CY vertically adjacent cells, so the tile is
+// TX x TH cells with TH = TY * RY * CY.  RY = 2 (two vertically adjacent outputs per thread, 13 % fewer shared-memory
+// loads per value, 217 registers, 8 warps) is bit-identical and was measured slower than RY = 1 with 12 warps.
 template <class T>
 struct TileShape;
 template <>
 struct TileShape<float> {
-    static constexpr int TX = 64, TY = 8, NS = 4, RY = 1;  // 16 warps x 128 registers, state in registers (4 stages: 4 % faster than 8)
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY * Arith<float>::CY;  // 12 warps, state in tensor memory
 };
 template <>
 struct TileShape<double> {
-    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1;  // 12 warps x 168 registers: window and delay line in tensor memory
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY;  // 12 warps x 168 registers: window and delay line in tensor memory
 };
 #ifndef FD6_V2_TY
 #define FD6_V2_TY 12
@@ -63,9 +71,10 @@ struct TileShape<double> {
 #endif
 template <>
 struct TileShape<V2> {
-    static constexpr int TX = 32, TY = FD6_V2_TY, NS = 4, RY = FD6_V2_RY;  // 12 warps x <= 168 registers: window and delay line in tensor memory
+    static constexpr int TX = 32, TY = FD6_V2_TY, NS = 4, RY = FD6_V2_RY, TH = TY * RY;  // 12 warps x <= 168 registers
 };
 
+// ---- host side -------------------------------------------------------------------------------------------
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                     const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
                                     CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -159,7 +168,7 @@ struct TiledTU {
     static cudaError_t set_smem(size_t bytes);            // opt every instantiation of this unit in to `bytes`
     static int max_ctas_per_sm(size_t bytes);             // occupancy of the fused kernel (the design assumes 1)
     // launches the instantiation for (path55, mode); false if there is none
-    static bool launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g, const KC<T>& c,
+    static bool launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g, const KC<typename Arith<T>::type>& c,
                        const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft);
 };
 
@@ -167,13 +176,13 @@ struct TiledTU {
 template <class T>
 inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
     ts.ready = false;
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, RY = TileShape<T>::RY;
+    constexpr int TX = TileShape<T>::TX, TH = TileShape<T>::TH;
     void* F[2] = {F0, F1};
     int rc = 0;
     for (int cur = 0; cur < 2 && rc == 0; ++cur) {
         Maps& m = ts.maps[cur];
-        rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TY * RY + 2 * R, 4);
-        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TY * RY, 4);
+        rc = tiled_make_map<T>(ts, &m.f_in, F[cur], g.px, g.py, g.pz, 4, g.px, g.py, g.fs, TX + 8, TH + 2 * R, 4);
+        if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TH, 4);
     }
     if (rc) return rc;
     const size_t smem = TiledTU<T, false>::smem_bytes(0);
@@ -195,7 +204,7 @@ inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
-    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TY * RY - 1) / (TY * RY), g.nz, ts.sm_count, &ts.items);
+    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TH - 1) / TH, g.nz, ts.sm_count, &ts.items);
     ts.ready = true;
     return 0;
 }
@@ -242,7 +251,7 @@ inline KC<T> make_kc(double dx, double nu, double cs, bool path55, double dt, do
 // Launch of the main kernel of one substep (fused 55-point kernel, or pass 1 of the 19-point path, which
 // leaves dt * div u in Div): reads copy `cur`, writes copy 1 - cur and w.
 template <class T>
-inline int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<T>& c,
+inline int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W, T* Div, const Geom& g, const KC<typename Arith<T>::type>& c,
                              const ForceTab<T>& ft, cudaStream_t stream) {
     const bool force = ft.tab != nullptr;
     if (force && !ts.force_fits) return 4;
