@@ -106,6 +106,12 @@ int fd_rhs(fd_ctx* ctx, void* d_lnrho, void* d_ux, void* d_uy, void* d_uz, int w
 /* Advance nsteps full RK3 steps (3 substeps each) of size dt.  FD_EINVAL: nsteps < 0 or dt not finite. */
 int fd_rk3_step(fd_ctx* ctx, double dt, int nsteps);
 
+/* fd_rk3_step enqueues each step as ONE CUDA graph launch (captured on first use, re-captured when dt, the path, the
+ * variant or the forcing changes) instead of its 6 (FD_PATH_55) or 15 (FD_PATH_19) kernel launches: the launch rate
+ * is what bounds small grids (BASELINE configs C1, C2).  on = 0 switches to plain launches; results are identical.
+ * With profiling on (fd_set_profiling) plain launches are used regardless.  Default: on. */
+int fd_set_graphs(fd_ctx* ctx, int on);
+
 /* Block until everything enqueued by this context has finished; returns FD_ECUDA if a kernel faulted. */
 int fd_sync(fd_ctx* ctx);
 

@@ -141,7 +141,7 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     const int n_full = (tiles / S) * S, rem = tiles - n_full;
     int best_k = 1;
     double best_cost = 1e300;
-    for (int k = 1; rem > 0 && k <= (nz + 7) / 8 && k <= 64; ++k) {
+    for (int k = 1; rem > 0 && k <= (nz + 1) / 2 && k <= 64; ++k) {  // chunks of >= 2 planes
         const int zc = (nz + k - 1) / k;
         const int real = (nz + zc - 1) / zc;
         const long long waves = ((long long)rem * real + S - 1) / S;

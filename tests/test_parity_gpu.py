@@ -345,7 +345,8 @@ def test_variant_switch_carries_a_loaded_state_across_layouts(mods):
     dt = 0.1 * dx
     F = smooth_state(rng, shape, 0.1, "f32")
     ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32)
-    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED  # AUTO: fp32, even nz
+    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_DIRECT  # AUTO on a tiny grid
+    ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)                   # fp32, even nz: the paired layout takes it
     ctx.load_state(F)
     order = [fd6.FD_VARIANT_TILED, fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_PAIRED, fd6.FD_VARIANT_DIRECT, fd6.FD_VARIANT_TILED]
     for n, v in enumerate(order, start=1):
@@ -373,6 +374,9 @@ def test_variant_switch_carries_a_loaded_state_across_layouts(mods):
 def test_paired_variant_is_refused_where_it_cannot_run(mods):
     O, fd6, I = mods
     ctx = fd6.Fd(16, 16, 9, 0.1, 0.01, 1.0, fd6.FD_F32)   # odd nz
+    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_DIRECT  # AUTO on a tiny grid
+    ctx.fd_destroy()
+    ctx = fd6.Fd(96, 96, 45, 0.1, 0.01, 1.0, fd6.FD_F32)  # odd nz, large enough for the staged kernels
     assert ctx.fd_get_info().variant == fd6.FD_VARIANT_TILED
     with pytest.raises(fd6.FdError) as e:
         ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)
@@ -406,3 +410,46 @@ def test_many_tiles_few_planes(mods, shape, dtype, path):
     ctx.fd_destroy()
     ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 1, path)
     assert relinf(got, ref) <= TOL[dtype], (wl.full_tiles, wl.chunks, wl.chunk_planes, wl.items)
+
+
+# ------------------------------------------------- CUDA-graph stepping (fd_set_graphs) against plain launches
+@pytest.mark.parametrize("dtype,shape", [("f32", (40, 26, 24)), ("f32", (40, 13, 9)), ("f64", (36, 20, 11))])
+@pytest.mark.parametrize("path", [0, 1])
+def test_graph_steps_equal_plain_launches_bitwise(mods, dtype, shape, path):
+    """One graph launch per step must enqueue exactly the launches of the plain path: same bits and the same launch
+    count, across an odd number of steps (the read copy alternates), a change of dt, of the forcing and of the variant
+    (each re-captures), and with the oracle as the referee of the whole trajectory."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(77 + path)
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.1, dtype)
+    kf, ef = (TWO_PI / (shape[0] * dx), 0.0, 2 * TWO_PI / (shape[2] * dx)), (0.0, 1.0, 0.0)
+
+    def trajectory(graphs):
+        ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32 if dtype == "f32" else fd6.FD_F64)
+        ctx.fd_set_path(path)
+        ctx.fd_set_graphs(graphs)
+        ctx.load_state(F)
+        n0 = ctx.fd_kernel_launches()
+        ctx.fd_rk3_step(dt, 3)
+        ctx.fd_rk3_step(dt, 2)
+        a = ctx.store_state()
+        ctx.fd_rk3_step(0.5 * dt, 1)
+        ctx.fd_set_forcing(kf, ef, 0.3, 0.02, dt)
+        ctx.fd_rk3_step(dt, 2)
+        ctx.fd_set_forcing(None, None, 0.0, 0.0, dt)
+        ctx.fd_set_variant(fd6.FD_VARIANT_DIRECT)
+        ctx.fd_rk3_step(dt, 1)
+        b = ctx.store_state()
+        n = ctx.fd_kernel_launches() - n0
+        ctx.fd_destroy()
+        return a, b, n
+
+    a1, b1, n1 = trajectory(True)
+    a0, b0, n0 = trajectory(False)
+    assert n1 == n0 and n1 > 0
+    assert all(np.array_equal(x, y) for x, y in zip(a1, a0))
+    assert all(np.array_equal(x, y) for x, y in zip(b1, b0))
+    ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 5, path)
+    assert relinf(a1, ref) <= 5 * TOL[dtype]
