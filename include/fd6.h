@@ -74,7 +74,8 @@ int fd_set_allocator(fd_alloc_fn alloc, fd_free_fn release, void* user);
 
 /* Create a context for an nx*ny*nz periodic grid, cell size dx (= dy = dz), viscosity nu, sound speed cs.
  * FD_EINVAL: out == NULL, any n < 8, dx <= 0, nu < 0, cs < 0, non-finite parameter, bad dtype.
- * FD_EUNSUPPORTED: nx % 4 != 0.  FD_ENOMEM / FD_ECUDA: allocation or CUDA failure (message in fd_last_error).
+ * FD_EUNSUPPORTED: nx % 4 != 0, ny > 65535, nz > 16383 or more than 2^33 cells.  FD_ENOMEM / FD_ECUDA: allocation or CUDA
+ * failure (message in fd_last_error).
  * The fields are zero (a uniform state at rest) until fd_load. */
 int fd_create(fd_ctx** out, int nx, int ny, int nz, double dx, double nu, double cs, int dtype);
 

@@ -284,7 +284,10 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
     T* W = (T*)c->W;
     T* Div = (T*)c->Div;
     const bool p55 = c->path == FD_PATH_55;
-    const bool tiled = c->variant == FD_VARIANT_TILED || c->variant == FD_VARIANT_PAIRED;
+    bool tiled = c->variant == FD_VARIANT_TILED || c->variant == FD_VARIANT_PAIRED;
+    // forcing on a grid whose z phase table does not fit beside the rings in shared memory: under AUTO the
+    // one-thread-per-cell kernels (which run on either layout) take the forced launches
+    if (tiled && c->force_on && !c->tiled.force_fits && c->variant_req == FD_VARIANT_AUTO) tiled = false;
     ForceTab<T> ft;
     ft.tab = c->force_on ? (const typename Scalar<T>::type*)c->ftab : nullptr;
     ft.nx = c->nx;
@@ -314,7 +317,7 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         LaunchScope ls(c, FD_K_PASS2);
         // y bands of 16 block rows once seven div planes no longer fit comfortably in L2 (see k_direct_pass2)
         const int brows = (g.ny + 3) / 4;
-        const bool banded = 7.0 * g.px * g.py * (double)c->esize > 32e6 && brows > 16;
+        const bool banded = 7.0 * g.px * g.py * (double)c->esize > 32e6 && brows > 16 && (long long)((brows + 15) / 16) * g.nz <= 65535;
         const int band_rows = banded ? 16 : brows, bands = (brows + band_rows - 1) / band_rows;
         dim3 grid2((g.nx + 63) / 64, band_rows, bands * g.nz);
         k_direct_pass2<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
@@ -619,6 +622,9 @@ extern "C" int fd_create(fd_ctx** out, int nx, int ny, int nz, double dx, double
     if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_create: bad dtype %d", dtype);
     if (nx % 4 != 0) return fail(FD_EUNSUPPORTED, "fd_create: nx must be a multiple of 4 (got %d)", nx);
     if ((long long)nx * ny * nz > (1LL << 33)) return fail(FD_EUNSUPPORTED, "fd_create: grid too large");
+    // launch grids put rows in gridDim.y and (field, plane) in gridDim.z, both limited to 65535
+    if (ny > 65535 || nz > 16383)
+        return fail(FD_EUNSUPPORTED, "fd_create: ny <= 65535 and nz <= 16383 (CUDA launch-grid limits; got ny %d, nz %d)", ny, nz);
     int ndev = 0;
     cudaError_t e = cudaGetDeviceCount(&ndev);
     if (e != cudaSuccess || ndev == 0) {

@@ -141,3 +141,31 @@ def test_forcing_argument_errors_on_a_live_context(mods):
     ctx.fd_rk3_step(0.01, 1)                       # and a failed call left the context usable
     assert np.array_equal(ctx.store_state(), np.zeros((4, 32, 32, 32), np.float32))
     ctx.fd_destroy()
+
+
+@pytest.mark.parametrize("path", [0, 1])
+def test_forcing_on_a_grid_too_deep_for_the_shared_z_table(mods, path):
+    """12000 planes: the forcing's z phase table no longer fits beside the staging rings of the staged kernels.  Under
+    FD_VARIANT_AUTO the forced launches fall back to the one-thread-per-cell kernels (no error, oracle parity); a variant
+    asked for by name still reports FD_EUNSUPPORTED."""
+    O, fd6, I = mods
+    shape = (32, 16, 12000)
+    rng = np.random.default_rng(12)
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.05, "f32")
+    sp = _spec(dt, k=(1.0, 0.5, 0.013), f0=0.05)
+    ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32)
+    ctx.fd_set_path(path)
+    assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED
+    ctx.load_state(F)
+    ctx.fd_set_forcing(sp["k"], sp["e"], sp["phi"], sp["f0"], sp["dt"])
+    ctx.fd_rk3_step(dt, 1)
+    got = ctx.store_state()
+    ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 1, path, force=sp)
+    assert relinf(got, ref) <= TOL["f32"]
+    ctx.fd_set_variant(fd6.FD_VARIANT_PAIRED)  # by name: the limit is reported
+    with pytest.raises(fd6.FdError) as e:
+        ctx.fd_rk3_step(dt, 1)
+    assert e.value.code == fd6.FD_EUNSUPPORTED
+    ctx.fd_destroy()

@@ -453,3 +453,27 @@ def test_graph_steps_equal_plain_launches_bitwise(mods, dtype, shape, path):
     assert all(np.array_equal(x, y) for x, y in zip(b1, b0))
     ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 5, path)
     assert relinf(a1, ref) <= 5 * TOL[dtype]
+
+
+# ------------------------------------------------- BASELINE config C2 as stated: 100 RK3 steps, both stencil paths
+@pytest.mark.parametrize("path", [0, 1])
+def test_c2_hundred_steps_full_grid_deviation_reported(mods, path, capsys):
+    """SURVEY 8(d), C2 row: after the config's own 100 steps the full-grid deviation from the oracle is REPORTED (printed;
+    DESIGN.md section 9 quotes it), not gated at the one-step tolerance: fp32 rounding differences between two correct
+    evaluation orders grow along the trajectory.  The gate here only catches a wrong trajectory (100 x the one-step bar)."""
+    O, fd6, I = mods
+    cfg = I.CONFIGS["C2"]
+    F = I.make_state(cfg)
+    ctx = fd6.Fd(cfg.n, cfg.n, cfg.n, cfg.dx, cfg.nu, cfg.cs, fd6.FD_F32)
+    ctx.fd_set_path(path)
+    ctx.load_state(F)
+    ctx.fd_rk3_step(cfg.dt, 100)
+    got = ctx.store_state()
+    variant = ctx.fd_get_info().variant
+    ctx.fd_destroy()
+    ref = O.rk3_step(F.astype(np.float64), cfg.dx, cfg.nu, cfg.cs, cfg.dt, 100, path)
+    dev = relinf(got, ref)
+    with capsys.disabled():
+        print(f"\nC2 128^3 fp32, 100 RK3 steps, {'55' if path == 0 else '19'}-point path, variant {variant}: "
+              f"max relative L-inf deviation from the fp64 oracle = {dev:.3e}")
+    assert dev <= 100 * TOL["f32"]
