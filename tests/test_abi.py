@@ -143,6 +143,18 @@ def test_work_list_of_the_headline_config(fd6):
     assert wl.chunks >= 2 and wl.items == 592 + 96 * wl.chunks
 
 
+def test_work_list_cuts_thin_grids_into_short_chunks(fd6):
+    """Few tiles and few stored planes: the remainder is cut down to chunks of a few planes (>= 2) so that its items fill
+    the SMs, in the paired layout too (round 1 capped the chunk count at planes / 8)."""
+    wl = fd6.fd_plan_work_list(132, 70, 20, fd6.FD_F32, 148)   # paired: 10 stored planes, 5 x 6 tiles
+    assert (wl.planes, wl.tiles_x * wl.tiles_y, wl.full_tiles) == (10, 30, 0)
+    assert wl.chunks >= 3 and 2 <= wl.chunk_planes <= 4 and wl.items <= 148
+    wl = fd6.fd_plan_work_list(2048, 100, 9, fd6.FD_F32, 148)  # plain fp32 (odd nz): 32 x 24 cells per tile
+    assert (wl.tile_x, wl.tile_y, wl.planes) == (32, 24, 9) and wl.chunks >= 2
+    wl = fd6.fd_plan_work_list(64, 64, 64, fd6.FD_F32, 148)
+    assert wl.chunks >= 8 and wl.chunk_planes >= 2
+
+
 def test_work_list_rejects_bad_arguments(fd6):
     wl = fd6.FdWorkList()
     assert fd6.lib.fd_plan_work_list(512, 512, 512, 0, 148, None) == fd6.FD_EINVAL
