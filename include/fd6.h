@@ -86,6 +86,13 @@ int fd_set_path(fd_ctx* ctx, int path);
 int fd_set_variant(fd_ctx* ctx, int variant);
 int fd_set_stream(fd_ctx* ctx, void* cuda_stream);
 
+/* Tile shape of the staged kernels (FD_VARIANT_TILED / FD_VARIANT_PAIRED): -1 automatic (default:
+ * by the number of tiles the grid gives), 0 "wide" (12 warps, one value per thread), 1 "tall" (8 warps, two vertically
+ * adjacent values per thread: fewer shared-memory loads per value, fewer and larger work items).  Results are bitwise
+ * identical; plain fp32 grids (odd nz) have the wide shape only and ignore the request.  Re-prepares the launches of the
+ * current variant.  FD_EINVAL: shape outside -1..1. */
+int fd_set_tile_shape(fd_ctx* ctx, int shape);
+
 /* Forcing term f of Eq. 2 (Eq. 24-25), frozen until the next call:
  *     f(x) = Re{ N f_k exp(i k.x + i phi) } = N f_k cos(k.x + phi),   x = (i, j, k) * dx (cell (0,0,0) at the origin),
  *     N = f0 cs sqrt(|k| cs / dt_ref),   f_k = (k x e) / sqrt(|k|^2 - (k.e)^2).

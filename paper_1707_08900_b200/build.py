@@ -5,9 +5,9 @@ Called by __graft_entry__.build().  Plain nvcc, static cudart, no libtorch: the 
 memory and streams through the hooks of fd6.h, so it does not depend on torch's ABI.
 
 Translation units (compiled in parallel, objects under paper_1707_08900_b200/build/, re-made only when a
-dependency or the flags changed): fd6.cu (C ABI, launch sequencing, the direct kernels) and six units of
-tiled-kernel instantiations, fd6_tiled_inst.cu for each value type (float, double, V2) with and without the
-forcing term.
+dependency or the flags changed): fd6.cu (C ABI, launch sequencing, the direct kernels) and ten units of
+tiled-kernel instantiations, fd6_tiled_inst.cu for each value type (float, double, V2), with and without the
+forcing term, in the wide and (double, V2) the tall tile shape.
 """
 import concurrent.futures
 import hashlib
@@ -37,10 +37,12 @@ _HEADERS = [os.path.join(INCLUDE, "fd6.h"), os.path.join(INCLUDE, "fd6_testing.h
 def units():
     """(object name, source, extra -D flags, dependencies)"""
     out = [("fd6.o", "fd6.cu", [], ["fd6.cu", "fd6_kernels_direct.cuh"] + _COMMON)]
-    for t in ("float", "double", "V2"):
-        for force in ("false", "true"):
-            out.append((f"tiled_{t}_{force}.o", "fd6_tiled_inst.cu", [f"-DFD6_INST_T={t}", f"-DFD6_INST_FORCE={force}"],
-                        ["fd6_tiled_inst.cu", "fd6_kernels_tiled.cuh"] + _COMMON))
+    for t, shapes in (("V2", (1, 0)), ("double", (1, 0)), ("float", (0,))):  # longest compilations first
+        for shape in shapes:
+            for force in ("false", "true"):
+                out.append((f"tiled_{t}_{force}_{shape}.o", "fd6_tiled_inst.cu",
+                            [f"-DFD6_INST_T={t}", f"-DFD6_INST_FORCE={force}", f"-DFD6_INST_SHAPE={shape}"],
+                            ["fd6_tiled_inst.cu", "fd6_kernels_tiled.cuh"] + _COMMON))
     return out
 
 
@@ -80,7 +82,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return obj, res
 
     failed = False
-    with concurrent.futures.ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+    with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as pool:
         for obj, res in pool.map(compile_one, jobs):
             if verbose or res.returncode != 0:
                 sys.stderr.write(f"---- {os.path.basename(obj)}\n" + res.stdout + res.stderr)

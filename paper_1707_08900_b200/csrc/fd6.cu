@@ -721,6 +721,16 @@ extern "C" int fd_set_variant(fd_ctx* c, int variant) {
     return rc;
 }
 
+extern "C" int fd_set_tile_shape(fd_ctx* c, int shape) {
+    FD_CHECK_CTX(c);
+    if (shape < -1 || shape > 1) return fail(FD_EINVAL, "fd_set_tile_shape: shape must be -1 (automatic), 0 (wide) or 1 (tall)");
+    const int old = c->tiled.shape_req;
+    c->tiled.shape_req = shape;
+    const int rc = resolve_variant(c);
+    if (rc) c->tiled.shape_req = old;
+    return rc;  // re-prepares the tensor maps and the work list of the current variant
+}
+
 extern "C" int fd_set_forcing(fd_ctx* c, const double* k, const double* e, double phi, double f0, double dt_ref) {
     FD_CHECK_CTX(c);
     if (!std::isfinite(f0) || f0 < 0) return fail(FD_EINVAL, "fd_set_forcing: f0 must be finite and >= 0");
@@ -891,17 +901,13 @@ extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count
     if (nx < 8 || ny < 8 || nz < 8 || sm_count < 1) return fail(FD_EINVAL, "fd_plan_work_list: bad grid or SM count");
     if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_plan_work_list: bad dtype %d", dtype);
     const bool paired = dtype == FD_F32 && nz % 2 == 0 && nz / 2 >= 4;  // what FD_VARIANT_AUTO resolves to
-    int tx, ty;
-    if (dtype == FD_F64) {
-        tx = TileShape<double>::TX;
-        ty = TileShape<double>::TH;
-    } else if (paired) {
-        tx = TileShape<V2>::TX;
-        ty = TileShape<V2>::TH;
-    } else {
-        tx = TileShape<float>::TX;
-        ty = TileShape<float>::TH;
-    }
+    int tx, ty;  // the tile shape tiled_prepare would pick for this grid
+    if (dtype == FD_F64)
+        shape_dims<double>(pick_shape<double>(nx, ny, sm_count, -1), &tx, &ty);
+    else if (paired)
+        shape_dims<V2>(pick_shape<V2>(nx, ny, sm_count, -1), &tx, &ty);
+    else
+        shape_dims<float>(0, &tx, &ty);
     const int planes = paired ? nz / 2 : nz;
     int items = 0;
     const Sched sc = plan_work_list((nx + tx - 1) / tx, (ny + ty - 1) / ty, planes, sm_count, &items);

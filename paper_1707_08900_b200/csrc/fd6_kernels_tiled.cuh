@@ -756,55 +756,56 @@ __global__ void __launch_bounds__(TX* TY, 1)
     Tiled<T, PATH55, TX, TY, NS, RY, FORCE, MODE>::run(m, g, c, sc, Fout, W, Div, ft);
 }
 
-// ---- TiledTU<T, FORCE>: the instantiations of one translation unit (see fd6_tiled_host.cuh) -------------------
+// ---- TiledTU<T, FORCE, S>: the instantiations of one translation unit (see fd6_tiled_host.cuh) ----------------
 // fn(kernel, path55, mode) for every instantiation of the main kernel of this unit.
-template <class T, bool FORCE, bool P55, int MODE, class Fn>
+template <class T, bool FORCE, int S, bool P55, int MODE, class Fn>
 static void each_kernel_1(Fn&& fn) {
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
-    fn(&k_tiled_main<T, P55, TX, TY, NS, RY, FORCE, MODE>, P55, MODE);
+    typedef TileShape<T, S> Sh;
+    fn(&k_tiled_main<T, P55, Sh::TX, Sh::TY, Sh::NS, Sh::RY, FORCE, MODE>, P55, MODE);
 }
-template <class T, bool FORCE, bool P55, class Fn>
+template <class T, bool FORCE, int S, bool P55, class Fn>
 static void each_kernel_2(Fn&& fn) {
-    each_kernel_1<T, FORCE, P55, 6>(fn);  // substep 1
-    each_kernel_1<T, FORCE, P55, 7>(fn);  // substep 2
-    each_kernel_1<T, FORCE, P55, 5>(fn);  // substep 3
-    each_kernel_1<T, FORCE, P55, 2>(fn);  // fd_rhs
+    each_kernel_1<T, FORCE, S, P55, 6>(fn);  // substep 1
+    each_kernel_1<T, FORCE, S, P55, 7>(fn);  // substep 2
+    each_kernel_1<T, FORCE, S, P55, 5>(fn);  // substep 3
+    each_kernel_1<T, FORCE, S, P55, 2>(fn);  // fd_rhs
 }
-template <class T, bool FORCE, class Fn>
+template <class T, bool FORCE, int S, class Fn>
 static void for_each_kernel(Fn&& fn) {
-    each_kernel_2<T, FORCE, true>(fn);
-    each_kernel_2<T, FORCE, false>(fn);
+    each_kernel_2<T, FORCE, S, true>(fn);
+    each_kernel_2<T, FORCE, S, false>(fn);
 }
 
-template <class T, bool FORCE>
-size_t TiledTU<T, FORCE>::smem_bytes(int planes) {  // the same for every instantiation of the unit
-    return Tiled<T, true, TileShape<T>::TX, TileShape<T>::TY, TileShape<T>::NS, TileShape<T>::RY, FORCE, 7>::smem_bytes(planes);
+template <class T, bool FORCE, int S>
+size_t TiledTU<T, FORCE, S>::smem_bytes(int planes) {  // the same for every instantiation of the unit
+    typedef TileShape<T, S> Sh;
+    return Tiled<T, true, Sh::TX, Sh::TY, Sh::NS, Sh::RY, FORCE, 7>::smem_bytes(planes);
 }
-template <class T, bool FORCE>
-cudaError_t TiledTU<T, FORCE>::set_smem(size_t bytes) {
+template <class T, bool FORCE, int S>
+cudaError_t TiledTU<T, FORCE, S>::set_smem(size_t bytes) {
     cudaError_t e = cudaSuccess;
-    for_each_kernel<T, FORCE>([&](auto kernel, bool, int) {
+    for_each_kernel<T, FORCE, S>([&](auto kernel, bool, int) {
         if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
     });
     return e;
 }
-template <class T, bool FORCE>
-int TiledTU<T, FORCE>::max_ctas_per_sm(size_t bytes) {
-    constexpr int TX = TileShape<T>::TX, TY = TileShape<T>::TY, NS = TileShape<T>::NS, RY = TileShape<T>::RY;
+template <class T, bool FORCE, int S>
+int TiledTU<T, FORCE, S>::max_ctas_per_sm(size_t bytes) {
+    typedef TileShape<T, S> Sh;
     int n = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_tiled_main<T, true, TX, TY, NS, RY, FORCE, 7>, TX * TY, bytes) != cudaSuccess) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, k_tiled_main<T, true, Sh::TX, Sh::TY, Sh::NS, Sh::RY, FORCE, 7>, Sh::TX * Sh::TY, bytes) !=
+        cudaSuccess) {
         cudaGetLastError();
         return -1;
     }
     return n;
 }
-template <class T, bool FORCE>
-bool TiledTU<T, FORCE>::launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g,
-                               const KC<typename Arith<T>::type>& c,
-                               const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft) {
-    dim3 block(TileShape<T>::TX, TileShape<T>::TY, 1), grid(items, 1, 1);
+template <class T, bool FORCE, int S>
+bool TiledTU<T, FORCE, S>::launch(bool path55, int mode, int items, size_t smem, cudaStream_t stream, const Maps& m, const Geom& g,
+                                  const KC<typename Arith<T>::type>& c, const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft) {
+    dim3 block(TileShape<T, S>::TX, TileShape<T, S>::TY, 1), grid(items, 1, 1);
     bool launched = false;
-    for_each_kernel<T, FORCE>([&](auto kernel, bool k55, int kmode) {
+    for_each_kernel<T, FORCE, S>([&](auto kernel, bool k55, int kmode) {
         if (!launched && k55 == path55 && kmode == mode) {
             kernel<<<grid, block, smem, stream>>>(m, g, c, sc, Fout, W, Div, ft);
             launched = true;

@@ -5,6 +5,7 @@
 #include <cuda.h>
 
 #include <cstdio>
+#include <type_traits>
 
 #include "fd6_common.cuh"
 
@@ -49,30 +50,62 @@ struct Maps {
 template <class T> struct Arith { typedef T type; static constexpr int CY = 1; };
 template <> struct Arith<float> { typedef V2 type; static constexpr int CY = 2; };
 
-// Tile shape per value type (registers per thread bound the CTA size).  TX x TY threads; a thread
-// owns RY columns of values, a value of the arithmetic type holds CY vertically adjacent cells, so the tile is
-// TX x TH cells with TH = TY * RY * CY.  RY = 2 (two vertically adjacent outputs per thread, 13 % fewer shared-memory
-// loads per value, 217 registers, 8 warps) is bit-identical and was measured slower than RY = 1 with 12 warps.
-template <class T>
+// Tile shapes (registers and tensor memory per thread bound the CTA size).  TX x TY threads; a
+// thread owns RY columns of values, a value of the arithmetic type holds CY vertically adjacent cells, so the tile is
+// TX x TH cells with TH = TY * RY * CY.  Two shapes, picked per grid by pick_shape():
+//   S = 0 "wide"  12 warps, one value per thread (32 x 12 values): 76 shared-memory loads per value
+//   S = 1 "tall"   8 warps, two vertically adjacent values per thread (32 x 16 values): the thread's x column is loaded
+//                 once for both (64 loads per value, bit-identical results); the state of two columns fills the tensor
+//                 memory of 2 warps per lane quadrant and ~230 registers.  Faster once a grid has enough tiles to fill
+//                 the SMs (C4: fused kernel -1.4 %, sustained +1.5 %, 20 % fewer shared-memory wavefronts); slower on
+//                 small grids, where fewer and larger tiles mean fewer work items (C2: +30 %).
+// Plain fp32 (y pairs) has the wide shape only.
+template <class T, int S>
 struct TileShape;
 template <>
-struct TileShape<float> {
-    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY * Arith<float>::CY;  // 12 warps, state in tensor memory
+struct TileShape<float, 0> {
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY * Arith<float>::CY;
 };
 template <>
-struct TileShape<double> {
-    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY;  // 12 warps x 168 registers: window and delay line in tensor memory
+struct TileShape<double, 0> {
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY;
 };
-#ifndef FD6_V2_TY
-#define FD6_V2_TY 12
-#endif
-#ifndef FD6_V2_RY
-#define FD6_V2_RY 1
-#endif
 template <>
-struct TileShape<V2> {
-    static constexpr int TX = 32, TY = FD6_V2_TY, NS = 4, RY = FD6_V2_RY, TH = TY * RY;  // 12 warps x <= 168 registers
+struct TileShape<double, 1> {
+    static constexpr int TX = 32, TY = 8, NS = 4, RY = 2, TH = TY * RY;
 };
+template <>
+struct TileShape<V2, 0> {
+    static constexpr int TX = 32, TY = 12, NS = 4, RY = 1, TH = TY * RY;
+};
+template <>
+struct TileShape<V2, 1> {
+    static constexpr int TX = 32, TY = 8, NS = 4, RY = 2, TH = TY * RY;
+};
+template <class T> struct Shapes { static constexpr int count = 2; };
+template <> struct Shapes<float> { static constexpr int count = 1; };
+
+// Shape for a grid: the tall one when its tiles give at least two thirds of an SM wave (measured: C3 with 128 tall
+// tiles on 148 SMs gains, C2 with 32 loses).  tile_h receives the tile height in stored values.
+template <class T>
+inline int pick_shape(int nx, int ny, int sm_count, int request) {
+    if (Shapes<T>::count < 2) return 0;
+    if (request >= 0) return request > 0 ? 1 : 0;
+    const long long tall = (long long)((nx + 31) / 32) * ((ny + 15) / 16);
+    return 3 * tall >= 2LL * sm_count ? 1 : 0;
+}
+template <class T>
+inline void shape_dims(int s, int* tx, int* th) {
+    if constexpr (Shapes<T>::count > 1) {
+        if (s == 1) {
+            *tx = TileShape<T, 1>::TX;
+            *th = TileShape<T, 1>::TH;
+            return;
+        }
+    }
+    *tx = TileShape<T, 0>::TX;
+    *th = TileShape<T, 0>::TH;
+}
 
 // ---- host side -------------------------------------------------------------------------------------------
 typedef CUresult (*PFN_encodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -85,6 +118,8 @@ struct TiledState {
     bool force_fits = true;  // the forcing's z table fits in shared memory beside the rings
     Sched sched{};     // work list
     int items = 0;     // grid size
+    int shape = 0;     // tile shape of the prepared launches (TileShape<T, shape>)
+    int shape_req = -1;  // -1: pick_shape decides; 0 / 1: forced (include/fd6_testing.h)
     int sm_count = 0;
     char err[256] = "";
 };
@@ -160,9 +195,9 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     return sc;
 }
 
-// The kernel instantiations of one value type live in translation units of their own (fd6_tiled_inst.cu, one per
-// value type and FORCE; compiled in parallel by build.py): this is the whole interface between them and fd6.cu.
-template <class T, bool FORCE>
+// The kernel instantiations of one (value type, FORCE, tile shape) live in a translation unit of their own
+// (fd6_tiled_inst.cu; compiled in parallel by build.py): this is the whole interface between them and fd6.cu.
+template <class T, bool FORCE, int S>
 struct TiledTU {
     static size_t smem_bytes(int planes);                 // dynamic shared memory of a launch over `planes` stored planes
     static cudaError_t set_smem(size_t bytes);            // opt every instantiation of this unit in to `bytes`
@@ -172,11 +207,9 @@ struct TiledTU {
                        const Sched& sc, T* Fout, T* W, T* Div, const ForceTab<T>& ft);
 };
 
-// F[0], F[1]: the two padded copies; W: the dense w arrays.
-template <class T>
-inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
-    ts.ready = false;
-    constexpr int TX = TileShape<T>::TX, TH = TileShape<T>::TH;
+template <class T, int S>
+inline int tiled_prepare_shape(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
+    constexpr int TX = TileShape<T, S>::TX, TH = TileShape<T, S>::TH;
     void* F[2] = {F0, F1};
     int rc = 0;
     for (int cur = 0; cur < 2 && rc == 0; ++cur) {
@@ -185,28 +218,39 @@ inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void
         if (rc == 0) rc = tiled_make_map<T>(ts, &m.w_ld, W, g.nx, g.ny, g.nz, 4, g.nx, g.ny, g.n, TX, TH, 4);
     }
     if (rc) return rc;
-    const size_t smem = TiledTU<T, false>::smem_bytes(0);
-    const size_t smem_f = TiledTU<T, true>::smem_bytes(g.nz);  // + the forcing's z table
+    const size_t smem = TiledTU<T, false, S>::smem_bytes(0);
+    const size_t smem_f = TiledTU<T, true, S>::smem_bytes(g.nz);  // + the forcing's z table
     ts.force_fits = smem_f <= 227 * 1024;
-    cudaError_t e = TiledTU<T, false>::set_smem(smem);
-    if (e == cudaSuccess && ts.force_fits) e = TiledTU<T, true>::set_smem(smem_f);
+    cudaError_t e = TiledTU<T, false, S>::set_smem(smem);
+    if (e == cudaSuccess && ts.force_fits) e = TiledTU<T, true, S>::set_smem(smem_f);
     if (e != cudaSuccess) {
         snprintf(ts.err, sizeof(ts.err), "cudaFuncSetAttribute(smem): %s", cudaGetErrorString(e));
         cudaGetLastError();
         return 3;
     }
     // the kernels take all of tensor memory and the work list counts waves of one CTA per SM
-    if (TiledTU<T, false>::max_ctas_per_sm(smem) != 1) {
+    if (TiledTU<T, false, S>::max_ctas_per_sm(smem) != 1) {
         snprintf(ts.err, sizeof(ts.err), "the tiled kernels are designed for exactly one resident CTA per SM");
         return 3;
     }
+    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TH - 1) / TH, g.nz, ts.sm_count, &ts.items);
+    ts.shape = S;
+    ts.ready = true;
+    return 0;
+}
+
+// F[0], F[1]: the two padded copies; W: the dense w arrays.
+template <class T>
+inline int tiled_prepare(TiledState& ts, const Geom& g, void* F0, void* F1, void* W) {
+    ts.ready = false;
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ts.sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (ts.sm_count <= 0) ts.sm_count = 148;
-    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TH - 1) / TH, g.nz, ts.sm_count, &ts.items);
-    ts.ready = true;
-    return 0;
+    if constexpr (Shapes<T>::count > 1) {
+        if (pick_shape<T>(g.nx, g.ny, ts.sm_count, ts.shape_req) == 1) return tiled_prepare_shape<T, 1>(ts, g, F0, F1, W);
+    }
+    return tiled_prepare_shape<T, 0>(ts, g, F0, F1, W);
 }
 
 inline const char* tiled_error_of(const TiledState& ts) { return ts.err; }
@@ -256,10 +300,22 @@ inline int tiled_launch_main(TiledState& ts, int path55, int cur, T* Fout, T* W,
     const bool force = ft.tab != nullptr;
     if (force && !ts.force_fits) return 4;
     const int mode = (c.read_w ? 1 : 0) | (c.write_w ? 2 : 0) | (c.write_f ? 4 : 0);
-    const bool launched = force ? TiledTU<T, true>::launch(path55 != 0, mode, ts.items, TiledTU<T, true>::smem_bytes(g.nz), stream, ts.maps[cur],
-                                                           g, c, ts.sched, Fout, W, Div, ft)
-                                : TiledTU<T, false>::launch(path55 != 0, mode, ts.items, TiledTU<T, false>::smem_bytes(0), stream, ts.maps[cur],
-                                                            g, c, ts.sched, Fout, W, Div, ft);
+    bool launched = false;
+    auto go = [&](auto shape_tag) {
+        constexpr int S = decltype(shape_tag)::value;
+        launched = force ? TiledTU<T, true, S>::launch(path55 != 0, mode, ts.items, TiledTU<T, true, S>::smem_bytes(g.nz), stream, ts.maps[cur], g,
+                                                       c, ts.sched, Fout, W, Div, ft)
+                         : TiledTU<T, false, S>::launch(path55 != 0, mode, ts.items, TiledTU<T, false, S>::smem_bytes(0), stream, ts.maps[cur], g,
+                                                        c, ts.sched, Fout, W, Div, ft);
+    };
+    if constexpr (Shapes<T>::count > 1) {
+        if (ts.shape == 1)
+            go(std::integral_constant<int, 1>());
+        else
+            go(std::integral_constant<int, 0>());
+    } else {
+        go(std::integral_constant<int, 0>());
+    }
     if (!launched) {
         snprintf(ts.err, sizeof(ts.err), "no tiled kernel for update mode %d", mode);
         return 3;

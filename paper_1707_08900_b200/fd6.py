@@ -25,7 +25,7 @@ EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
     "fd_rhs", "fd_rk3_step", "fd_sync", "fd_destroy", "fd_last_error", "fd_get_info", "fd_kernel_launches",
     "fd_set_profiling", "fd_get_profile", "fd_reset_profile",
-    "fd_plan_work_list", "fd_set_forcing", "fd_set_graphs",
+    "fd_plan_work_list", "fd_set_forcing", "fd_set_graphs", "fd_set_tile_shape",
 ]
 
 if not os.path.exists(_LIB_PATH):
@@ -71,6 +71,7 @@ lib.fd_set_profiling.argtypes = [_vp, _i]
 lib.fd_get_profile.argtypes = [_vp, _i, C.POINTER(_d), C.POINTER(C.c_ulonglong)]
 lib.fd_reset_profile.argtypes = [_vp]
 lib.fd_set_graphs.argtypes = [_vp, _i]
+lib.fd_set_tile_shape.argtypes = [_vp, _i]
 lib.fd_set_forcing.argtypes = [_vp, C.POINTER(_d), C.POINTER(_d), _d, _d, _d]
 lib.fd_plan_work_list.argtypes = [_i, _i, _i, _i, _i, C.POINTER(FdWorkList)]
 
@@ -161,6 +162,10 @@ class Fd:
     def fd_set_variant(self, variant):
         self._stream()  # a switch of layout converts the resident state on the stream
         _check(lib.fd_set_variant(self._h, variant))
+
+    def fd_set_tile_shape(self, shape):
+        self._stream()
+        _check(lib.fd_set_tile_shape(self._h, int(shape)))
 
     def fd_set_graphs(self, on):
         _check(lib.fd_set_graphs(self._h, int(bool(on))))

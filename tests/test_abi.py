@@ -138,9 +138,15 @@ def test_work_list_covers_every_tile_plane_exactly_once(fd6, shape, dtype, sms):
 
 def test_work_list_of_the_headline_config(fd6):
     wl = fd6.fd_plan_work_list(512, 512, 512, fd6.FD_F32, 148)
-    # 16 x 43 tiles of 32 x 12 pairs: four full waves of columns, the remaining 96 tiles cut in z
-    assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes, wl.full_tiles) == (32, 12, 16, 43, 256, 592)
-    assert wl.chunks >= 2 and wl.items == 592 + 96 * wl.chunks
+    # enough tiles for the tall shape: 16 x 32 tiles of 32 x 16 pairs; three full waves of columns, the remaining 68
+    # tiles cut in z
+    assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes, wl.full_tiles) == (32, 16, 16, 32, 256, 444)
+    assert wl.chunks >= 2 and wl.items == 444 + 68 * wl.chunks
+    # a grid with few tiles keeps the wide shape (32 x 12 values): more, smaller work items
+    wl = fd6.fd_plan_work_list(128, 128, 128, fd6.FD_F32, 148)
+    assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes) == (32, 12, 4, 11, 64)
+    wl = fd6.fd_plan_work_list(256, 256, 256, fd6.FD_F64, 148)
+    assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes) == (32, 16, 8, 16, 256)
 
 
 def test_work_list_cuts_thin_grids_into_short_chunks(fd6):

@@ -477,3 +477,34 @@ def test_c2_hundred_steps_full_grid_deviation_reported(mods, path, capsys):
         print(f"\nC2 128^3 fp32, 100 RK3 steps, {'55' if path == 0 else '19'}-point path, variant {variant}: "
               f"max relative L-inf deviation from the fp64 oracle = {dev:.3e}")
     assert dev <= 100 * TOL["f32"]
+
+
+# ------------------------------------------------- the two tile shapes of the staged kernels (fd_set_tile_shape)
+@pytest.mark.parametrize("shape", [(40, 13, 10), (132, 70, 20), (72, 33, 42), (512, 500, 16), (36, 1000, 10), (132, 2000, 12)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("path", [0, 1])
+def test_tall_tiles_equal_wide_tiles_bitwise(mods, shape, dtype, path):
+    """The tall shape (two vertically adjacent values per thread) loads less but computes every value with the same
+    operations in the same order as the wide one: identical bits, on ragged grids, on grids with many tiles and few planes
+    (z-chunked remainders), for the paired fp32 and the fp64 kernels, on both paths; and both within the one-step bar."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(sum(shape) + path)
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.1, dtype)
+    out = []
+    for tile_shape in (0, 1):
+        ctx = make_ctx(fd6, shape, dx, nu, cs, dtype, path, fd6.FD_VARIANT_PAIRED if dtype == "f32" else fd6.FD_VARIANT_TILED)
+        ctx.fd_set_tile_shape(tile_shape)
+        T.fd_debug_poison_ghosts(ctx)
+        ctx.load_state(F)
+        T.fd_debug_poison_w(ctx)
+        ctx.fd_rk3_step(dt, 2)
+        out.append(ctx.store_state())
+        R = ctx.rhs_state()
+        out.append(R)
+        ctx.fd_destroy()
+    assert all(np.array_equal(a, b) for a, b in zip(out[0], out[2]))
+    assert all(np.array_equal(a, b) for a, b in zip(out[1], out[3]))
+    ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 2, path)
+    assert relinf(out[2], ref) <= 2 * TOL[dtype]
