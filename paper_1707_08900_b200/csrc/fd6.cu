@@ -9,6 +9,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <type_traits>
 #include <vector>
 
 #include "fd6_common.cuh"
@@ -319,8 +320,13 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         const int brows = (g.ny + 3) / 4;
         const bool banded = 7.0 * g.px * g.py * (double)c->esize > 32e6 && brows > 16 && (long long)((brows + 15) / 16) * g.nz <= 65535;
         const int band_rows = banded ? 16 : brows, bands = (brows + band_rows - 1) / band_rows;
-        dim3 grid2((g.nx + 63) / 64, band_rows, bands * g.nz);
-        k_direct_pass2<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+        if constexpr (std::is_same<T, float>::value) {  // plain fp32: two x-adjacent cells per thread
+            dim3 grid2((g.nx + 127) / 128, band_rows, bands * g.nz);
+            k_direct_pass2_x2<<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+        } else {
+            dim3 grid2((g.nx + 63) / 64, band_rows, bands * g.nz);
+            k_direct_pass2<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
+        }
     }
     FD_CUDA(cudaGetLastError());
     if (s.write_f) {
