@@ -82,6 +82,11 @@ def test_argument_validation_happens_before_any_cuda_call(fd6):
     assert L.fd_create(C.byref(h), 32, 32, 32, 0.1, 0.0, -1.0, fd6.FD_F32) == fd6.FD_EINVAL
     assert L.fd_create(C.byref(h), 32, 32, 32, 0.1, 0.0, 1.0, 7) == fd6.FD_EINVAL
     assert L.fd_create(C.byref(h), 30, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32) == fd6.FD_EUNSUPPORTED
+    # launch-grid limits (rows in gridDim.y, (field, plane) in gridDim.z): refused up front, not at the first launch
+    assert L.fd_create(C.byref(h), 32, 70000, 8, 0.1, 0.0, 1.0, fd6.FD_F64) == fd6.FD_EUNSUPPORTED
+    assert L.fd_create(C.byref(h), 32, 8, 16384, 0.1, 0.0, 1.0, fd6.FD_F64) == fd6.FD_EUNSUPPORTED
+    assert b"launch-grid" in L.fd_last_error()
+    assert L.fd_set_tile_shape(None, 0) == fd6.FD_EINVAL and L.fd_set_graphs(None, 1) == fd6.FD_EINVAL
     assert h.value is None
     # NULL context
     assert L.fd_rk3_step(None, 0.1, 1) == fd6.FD_EINVAL
