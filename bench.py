@@ -220,6 +220,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 direct, 2 tiled, 3 paired")
     ap.add_argument("--tile-shape", type=int, default=-1, help="-1 automatic, 0 wide (12 warps), 1 tall (8 warps x 2 values)")
+    ap.add_argument("--tile-overlap", type=int, default=0,
+                    help="measurement aid (include/fd6_testing.h): tiles overlap by this many values, same results, the redundant "
+                         "halo-ring work of temporal blocking (DESIGN.md section 7)")
     ap.add_argument("--forcing", action="store_true",
                     help="switch the forcing term of Eq. 2 on (Eq. 24-25; off in the paper's performance runs, PAPER.md:369)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -263,6 +266,9 @@ def main():
         ctx.fd_set_variant(args.variant)
     if args.tile_shape >= 0:
         ctx.fd_set_tile_shape(args.tile_shape)
+    if args.tile_overlap:
+        from paper_1707_08900_b200 import fd6_testing
+        fd6_testing.fd_debug_set_tile_overlap(ctx, args.tile_overlap)
     info = ctx.fd_get_info()
     wl = fd6.fd_plan_work_list(n, n, n, fd6.FD_F32 if cfg.dtype == "f32" else fd6.FD_F64, 148)
     tile = {0: "wide 32x12", 1: "tall 32x16"}.get(args.tile_shape, f"automatic ({wl.tile_x}x{wl.tile_y})") if info.variant in (2, 3) else None
@@ -362,7 +368,7 @@ def main():
     actual = DOMINANT_WORDS_ACTUAL_MEAN[args.path] * esize * N / avg_launch_s / 1e9 if dom_n else None
     kern_share = {k: round(v[0] / prof_ms, 4) for k, v in prof.items() if v[1]}
     variant_name = {1: "direct", 2: "tiled", 3: "paired"}.get(info.variant, str(info.variant))
-    ncu = (ncu_entry(args.config, dom, variant_name) or {}) if args.tile_shape < 0 else {}
+    ncu = (ncu_entry(args.config, dom, variant_name) or {}) if args.tile_shape < 0 and not args.tile_overlap else {}
     step_gbs = WORDS_PER_CELL_SUBSTEP[args.path] * esize * 3 * N * K / (ms_max * 1e-3) / 1e9
     step_gbs_actual = WORDS_PER_CELL_STEP_ACTUAL[args.path] * esize * N * K / (ms_max * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
@@ -392,7 +398,7 @@ def main():
             "dtype": cfg.dtype, "data": "synthetic",
             "config": {"workload": f"{cfg.name}: {n}^3 periodic {cfg.dtype}, band-limited |k|<={cfg.kmax} rms Mach {cfg.amp}, "
                                    f"nu={cfg.nu}, dt=0.1 dx/cs", "path": f"{args.path}-point",
-                       "variant": variant_name, "tile_shape": tile,
+                       "variant": variant_name, "tile_shape": tile, "tile_overlap": args.tile_overlap,
                        "l2": l2_note, "launch": "one CUDA graph per RK3 step (fd_set_graphs on)",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite,
                        "forcing": (f"on: k={forcing['k']}, f0={forcing['f0']}" if forcing else "off (PAPER.md:369)")},

@@ -21,6 +21,13 @@ int fd_debug_poison_w(fd_ctx* ctx);
  * context as holding a non-zero state.  FD_EINVAL: ctx == NULL. */
 int fd_debug_poison_ghosts(fd_ctx* ctx);
 
+/* Measurement aid for DESIGN.md section 7 ("temporal blocking"): let neighbouring tiles of the staged kernels overlap by
+ * `overlap` values in x and y (even, smaller than the tile; 0 = off, the product setting).  Every tile is still evaluated
+ * in full, a value is stored by the tile that holds it furthest from its edge, so results are unchanged (bitwise) while
+ * the launch does the redundant halo-ring work that the first of two fused substeps would have to do (overlap 6 = a
+ * radius-3 ring).  fp64 and the paired fp32 layout only.  FD_EINVAL / FD_ECUDA with a message otherwise. */
+int fd_debug_set_tile_overlap(fd_ctx* ctx, int overlap);
+
 #ifdef __cplusplus
 }
 #endif

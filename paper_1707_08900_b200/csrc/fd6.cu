@@ -954,6 +954,19 @@ extern "C" int fd_debug_poison_w(fd_ctx* c) {
     return FD_DISPATCH(c, do_poison<T>(c, false));
 }
 
+extern "C" int fd_debug_set_tile_overlap(fd_ctx* c, int overlap) {
+    FD_CHECK_CTX(c);
+    if (overlap < 0) return fail(FD_EINVAL, "fd_debug_set_tile_overlap: overlap < 0");
+    const int old = c->tiled.overlap;
+    c->tiled.overlap = overlap;
+    const int rc = resolve_variant(c);
+    if (rc) {
+        c->tiled.overlap = old;
+        resolve_variant(c);
+    }
+    return rc;
+}
+
 extern "C" int fd_debug_poison_ghosts(fd_ctx* c) {
     FD_CHECK_CTX(c);
     return FD_DISPATCH(c, do_poison<T>(c, true));

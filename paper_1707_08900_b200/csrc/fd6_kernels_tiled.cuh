@@ -585,7 +585,8 @@ struct Tiled {
             ze = min(zs + sc.zc, g.nz);
         }
         if (zs >= ze) return;  // empty chunk (rounding); the whole CTA leaves before any barrier
-        const int X0 = (tile % sc.ntx) * TX, Y0 = (tile / sc.ntx) * TH;
+        const int tbx = tile % sc.ntx, tby = tile / sc.ntx;
+        const int X0 = tbx * (TX - sc.ov), Y0 = tby * (TH - sc.ov);  // ov = 0 except in the temporal-blocking emulation
         const int np = ze - zs + 2 * R;  // staged planes t = zs-3 .. ze+2
         constexpr int L = Scalar<T>::lanes;
         // TMA box origin; the tensor maps count scalars along x, a value is L of them
@@ -641,7 +642,16 @@ struct Tiled {
         bool ok[RY];
 #pragma unroll
         for (int r = 0; r < RY; ++r) ok[r] = ci < g.nx && cj + r < g.ny;
-        const bool store_ok = ok[0];
+        if (sc.ov > 0) {  // overlapping tiles: a value is stored by the tile whose interior (edge minus ov / 2) holds it
+            const int h = sc.ov / 2;
+            const bool in_x = (tbx == 0 || tx >= h) && (tbx == sc.ntx - 1 || tx < TX - h);
+#pragma unroll
+            for (int r = 0; r < RY; ++r) {
+                const int row = ty * RY + r;
+                ok[r] = ok[r] && in_x && (tby == 0 || row >= h) && (tby == sc.nty - 1 || row < TH - h);
+            }
+        }
+        const bool store_ok = ci < g.nx && cj < g.ny;  // the thread's first cell is inside the grid: its offsets are valid
         const bool okb = YP && ci < g.nx && cj + 1 < g.ny;  // y pairs: the second cell of the thread is inside the grid
         if constexpr (FORCE && TM) {
 #pragma unroll

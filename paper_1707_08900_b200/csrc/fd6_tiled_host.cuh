@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <type_traits>
 
@@ -35,6 +36,10 @@ struct Sched {
     int ntx;     // tiles along x; tile index = bx + ntx * by
     int n_full;  // tiles with a single item
     int k, zc;   // chunks per remaining tile, planes per chunk
+    int nty;     // tiles along y
+    int ov;      // 0, or (include/fd6_testing.h, fd_debug_set_tile_overlap) the number of values by which neighbouring tiles
+                 // overlap in x and y: every tile is still computed in full, a value is stored by the tile that holds it
+                 // furthest from its edge.  Emulates the redundant halo-ring evaluation of temporal blocking (DESIGN 7).
 };
 
 // The tensor maps of one launch (each 128 bytes, passed by value as a __grid_constant__ parameter).
@@ -119,7 +124,8 @@ struct TiledState {
     Sched sched{};     // work list
     int items = 0;     // grid size
     int shape = 0;     // tile shape of the prepared launches (TileShape<T, shape>)
-    int shape_req = -1;  // -1: pick_shape decides; 0 / 1: forced (include/fd6_testing.h)
+    int shape_req = -1;  // -1: pick_shape decides; 0 / 1: forced (fd_set_tile_shape)
+    int overlap = 0;     // tile overlap of the temporal-blocking emulation (include/fd6_testing.h); 0 in every product launch
     int sm_count = 0;
     char err[256] = "";
 };
@@ -188,6 +194,8 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     }
     Sched sc;
     sc.ntx = ntx;
+    sc.nty = nty;
+    sc.ov = 0;
     sc.n_full = n_full;
     sc.zc = (nz + best_k - 1) / best_k;
     sc.k = (nz + sc.zc - 1) / sc.zc;
@@ -233,7 +241,16 @@ inline int tiled_prepare_shape(TiledState& ts, const Geom& g, void* F0, void* F1
         snprintf(ts.err, sizeof(ts.err), "the tiled kernels are designed for exactly one resident CTA per SM");
         return 3;
     }
-    ts.sched = plan_work_list((g.nx + TX - 1) / TX, (g.ny + TH - 1) / TH, g.nz, ts.sm_count, &ts.items);
+    const int ov = ts.overlap;
+    if (ov > 0 && (Arith<T>::CY != 1 || ov % 2 != 0 || ov >= TX || ov >= TH)) {
+        snprintf(ts.err, sizeof(ts.err), "tile overlap: even, smaller than the tile, 8-byte value types only");
+        return 3;
+    }
+    // tiles step by (TX - ov, TH - ov); the last tile of a row / column may hang over the grid (clipped as usual)
+    const int ntx = ov ? (std::max(g.nx - ov, 1) + (TX - ov) - 1) / (TX - ov) : (g.nx + TX - 1) / TX;
+    const int nty = ov ? (std::max(g.ny - ov, 1) + (TH - ov) - 1) / (TH - ov) : (g.ny + TH - 1) / TH;
+    ts.sched = plan_work_list(ntx, nty, g.nz, ts.sm_count, &ts.items);
+    ts.sched.ov = ov;
     ts.shape = S;
     ts.ready = true;
     return 0;

@@ -508,3 +508,28 @@ def test_tall_tiles_equal_wide_tiles_bitwise(mods, shape, dtype, path):
     assert all(np.array_equal(a, b) for a, b in zip(out[1], out[3]))
     ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 2, path)
     assert relinf(out[2], ref) <= 2 * TOL[dtype]
+
+
+@pytest.mark.parametrize("shape", [(132, 70, 20), (72, 33, 42), (512, 500, 16)])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("tile_shape", [0, 1])
+def test_overlapping_tiles_give_the_same_bits(mods, shape, dtype, tile_shape):
+    """fd_debug_set_tile_overlap (the temporal-blocking emulation DESIGN.md section 7 measures): tiles that overlap by a
+    radius-3 ring on every side do redundant work but store every value exactly once, with unchanged bits."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(sum(shape))
+    dx, nu, cs = 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(rng, shape, 0.1, dtype)
+    out = []
+    for overlap in (0, 6):
+        ctx = make_ctx(fd6, shape, dx, nu, cs, dtype, 0, fd6.FD_VARIANT_PAIRED if dtype == "f32" else fd6.FD_VARIANT_TILED)
+        ctx.fd_set_tile_shape(tile_shape)
+        T.fd_debug_set_tile_overlap(ctx, overlap)
+        ctx.load_state(F)
+        ctx.fd_rk3_step(dt, 2)
+        out.append(ctx.store_state())
+        ctx.fd_destroy()
+    assert all(np.array_equal(a, b) for a, b in zip(out[0], out[1]))
+    ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 2, 0)
+    assert relinf(out[1], ref) <= 2 * TOL[dtype]
