@@ -268,8 +268,13 @@ static int launch_halo(fd_ctx* c, T* F, int nfields) {
     LaunchScope ls(c, FD_K_HALO);
     const int yz_rows = 2 * R * g.py + 2 * R * g.nz;
     const long long xthreads = 2LL * g.ny * g.nz * nfields;
-    const long long blocks = (long long)nfields * yz_rows + (xthreads + 127) / 128;
-    k_halo<T><<<(unsigned)blocks, 128, 0, c->stream>>>(F, g, nfields, yz_rows);
+    // several ghost rows per block when a row has fewer 32-byte sectors than a block has threads (narrow grids)
+    const int nsec = g.nx / g.gx + 2;
+    int rpb = 1;
+    while (rpb < 8 && 128 / (2 * rpb) >= nsec) rpb *= 2;
+    const long long row_blocks = ((long long)nfields * yz_rows + rpb - 1) / rpb;
+    const long long blocks = row_blocks + (xthreads + 127) / 128;
+    k_halo<T><<<(unsigned)blocks, 128, 0, c->stream>>>(F, g, nfields, yz_rows, rpb, (int)row_blocks);
     FD_CUDA(cudaGetLastError());
     return FD_OK;
 }

@@ -55,7 +55,8 @@ __global__ void __launch_bounds__(128)
 // a1 / a7  periodic halo fill, radius 3 (Alg. 2/3 "Compute boundary conditions").
 //   (T = V2: the stored grid has nz/2 planes and z-periodicity swaps the halves of a pair, see zwrap.)
 //   One kernel, every ghost value read straight from the interior (no ordering between faces):
-//   blocks [0, nfields * yz_rows): one ghost ROW each (j or k outside the domain) = the x-extended copy of the
+//   blocks [0, row_blocks): `rpb` ghost ROWS each (rpb > 1 on narrow grids, where a row has fewer sectors than the block has
+//       threads; row index in [0, nfields * yz_rows)); a ghost row (j or k outside the domain) = the x-extended copy of the
 //       interior row it wraps to, its own 2R x ghosts taken from the far end of that row; this also fills the
 //       edge ghosts (two coordinates outside) the Eq. 8 diagonals read, and the corners (never read);
 //   remaining blocks: the x ghosts of the interior rows, one thread per (row, side): the x ghost pad is exactly one
@@ -63,11 +64,14 @@ __global__ void __launch_bounds__(128)
 //       [0, gx) takes the last gx interior values, the high pad the first gx (only R of them are ever read).
 // ------------------------------------------------------------------------------------------------
 template <class T>
-__global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfields, int yz_rows) {
-    if ((int)blockIdx.x < nfields * yz_rows) {
+__global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfields, int yz_rows, int rpb, int row_blocks) {
+    if ((int)blockIdx.x < row_blocks) {
         // ghost rows: first the 2R ghost z-planes (py rows each), then for every interior plane its 2R ghost y-rows
-        const int q = blockIdx.x / yz_rows;
-        int b = blockIdx.x - q * yz_rows, jj, kk;
+        const int tpr = 128 / rpb;  // threads per row
+        const int row = blockIdx.x * rpb + threadIdx.x / tpr, lane = threadIdx.x - (threadIdx.x / tpr) * tpr;
+        if (row >= nfields * yz_rows) return;
+        const int q = row / yz_rows;
+        int b = row - q * yz_rows, jj, kk;
         const int zrows = 2 * R * g.py;
         if (b < zrows) {
             int zp = b / g.py;
@@ -92,7 +96,7 @@ __global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfi
             // whole 32-byte sectors (gx values): sector 0 is the low pad, the last one the high pad
             constexpr int VPS = (int)(32 / sizeof(T));  // == g.gx
             const int nsec = g.nx / VPS + 2;
-            for (int sct = threadIdx.x; sct < nsec; sct += 128) {
+            for (int sct = lane; sct < nsec; sct += tpr) {
                 const int ssrc = sct == 0 ? nsec - 2 : (sct == nsec - 1 ? 1 : sct);
                 union { uint4 u[2]; T v[VPS]; } buf;
                 const uint4* sp = reinterpret_cast<const uint4*>(srow + ssrc * VPS);
@@ -109,7 +113,7 @@ __global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfi
         } else {
             T* dst = drow + (g.gx - R);
             const T* src = srow + (g.gx - R);
-            for (int x = threadIdx.x; x < g.nx + 2 * R; x += 128) {
+            for (int x = lane; x < g.nx + 2 * R; x += tpr) {
                 const int xs = x < R ? x + g.nx : (x >= g.nx + R ? x - g.nx : x);
                 const T v = src[xs];
                 dst[x] = zw ? zwrap<T>(v) : v;
@@ -117,7 +121,7 @@ __global__ void __launch_bounds__(128) k_halo(T* __restrict__ F, Geom g, int nfi
         }
         return;
     }
-    long long t = (long long)(blockIdx.x - nfields * yz_rows) * 128 + threadIdx.x;
+    long long t = (long long)(blockIdx.x - row_blocks) * 128 + threadIdx.x;
     const int side = (int)(t & 1);
     t >>= 1;
     long long rows = (long long)g.ny * g.nz;
