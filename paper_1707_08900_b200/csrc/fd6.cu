@@ -964,7 +964,11 @@ extern "C" int fd_debug_set_tile_overlap(fd_ctx* c, int overlap) {
     if (overlap < 0) return fail(FD_EINVAL, "fd_debug_set_tile_overlap: overlap < 0");
     const int old = c->tiled.overlap;
     c->tiled.overlap = overlap;
-    const int rc = resolve_variant(c);
+    int rc = resolve_variant(c);
+    // under AUTO a refused overlap would silently fall back to the direct kernels: report it instead
+    if (rc == FD_OK && overlap > 0 && c->variant != FD_VARIANT_TILED && c->variant != FD_VARIANT_PAIRED)
+        rc = fail(FD_EUNSUPPORTED, "fd_debug_set_tile_overlap: the staged kernels do not run this grid with overlap %d (%s)", overlap,
+                  tiled_error_of(c->tiled));
     if (rc) {
         c->tiled.overlap = old;
         resolve_variant(c);
