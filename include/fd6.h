@@ -111,6 +111,49 @@ int fd_store(fd_ctx* ctx, void* lnrho, void* ux, void* uy, void* uz, int where);
  * state is not changed. */
 int fd_rhs(fd_ctx* ctx, void* d_lnrho, void* d_ux, void* d_uy, void* d_uz, int where);
 
+/* fd_rhs_static — the right-hand side of Eq. 1-3 by the fused 55-point stencil (Eq. 6-8, Alg. 2,
+ * PAPER.md:97-108, 207-213) for callers that cannot allocate device memory.
+ *
+ * Why it exists.  Everything else in this header goes through fd_create, which allocates the ghost-padded field copies
+ * and the w arrays (cudaMalloc, or the fd_set_allocator hook).  Some users of the library are not in a position to do
+ * that: a solver plug-in inside an application that has given all device memory to its own pool and forbids further
+ * driver allocations; a time loop that may not touch cudaMalloc / cudaFree because both synchronise the whole device and
+ * stall every other stream; a job running so close to the memory limit that a late allocation could fail.  For them
+ * this one call needs no context and allocates nothing — no cudaMalloc, no cudaFree, no allocating library routine:
+ * the ghost-padded copy of the state that the stencil kernel reads lives in a fixed array inside libfd6.so itself.
+ *
+ * The price.  That array is FD_RHS_STATIC_MAX_BYTES (8 MiB) of device memory which every GPU that loads the library
+ * keeps until the process exits, used or not, and it bounds the grid: the padded state, 4 fields of
+ * px * (ny + 6) * (nz + 6) values (rounded up to a multiple of 256 bytes per field) with
+ * px = nx + 16 rounded up to a multiple of 8 (FD_F32) or nx + 8 rounded up to a multiple of 4 (FD_F64), must fit —
+ * e.g. up to 64^3 in FD_F32 or 48^3 in FD_F64 (BASELINE config C1, 32^3 FD_F64, takes 1.8 MiB).  Larger grids are
+ * refused with FD_EUNSUPPORTED and a message that states both sizes; use fd_create + fd_rhs for them.
+ *
+ * Arguments.  nx, ny, nz, dx, nu, cs, dtype as for fd_create (same checks, same error codes).  lnrho, ux, uy, uz: the
+ * state, and d_lnrho, d_ux, d_uy, d_uz: the result, are eight dense DEVICE arrays of nx*ny*nz elements in the layout
+ * of "Conventions" above, owned by the caller, on the CURRENT device (the caller makes the device of its pointers and
+ * of `cuda_stream` current before the call); the result arrays must not overlap each other or the state.  cuda_stream
+ * is a cudaStream_t passed as void* (NULL = legacy default stream).  Three kernels are enqueued on it (copy into the
+ * padded scratch, periodic halo fill, stencil + assembly straight into the result arrays) and the call returns without
+ * waiting.  No forcing term.  Results agree with fd_rhs on FD_PATH_55 to rounding (same formulas and coefficients).
+ *
+ * First call on a device.  The first call on each device looks up the device address of the built-in array (once; this
+ * may load the library's kernels onto that device).  Make that first call before starting any stream capture.
+ *
+ * Sharing.  All calls on a device use the same array, and it keeps whatever the last call left in it.  Nothing in it
+ * has to start from zero: every value the stencil kernel reads is rewritten by the copy-in and the halo fill of the
+ * same call (a test runs a small grid after a large one to show stale contents do not leak).  But two calls whose
+ * kernels can overlap on the GPU — different streams without an ordering between them, or different host threads —
+ * race on the array and give wrong results: keep the calls of one device on one stream, or order them with events.
+ *
+ * FD_EINVAL: a NULL pointer, any n < 8, dx <= 0, nu < 0, cs < 0, a non-finite parameter, bad dtype.
+ * FD_EUNSUPPORTED: nx % 4 != 0, or the padded state exceeds FD_RHS_STATIC_MAX_BYTES.  FD_ECUDA: no device, the address
+ * look-up or a launch failed (message in fd_last_error).  Argument errors are reported before any CUDA call. */
+#define FD_RHS_STATIC_MAX_BYTES (8u * 1024u * 1024u)
+int fd_rhs_static(int nx, int ny, int nz, double dx, double nu, double cs, int dtype,
+                  const void* lnrho, const void* ux, const void* uy, const void* uz,
+                  void* d_lnrho, void* d_ux, void* d_uy, void* d_uz, void* cuda_stream);
+
 /* Advance nsteps full RK3 steps (3 substeps each) of size dt.  FD_EINVAL: nsteps < 0 or dt not finite. */
 int fd_rk3_step(fd_ctx* ctx, double dt, int nsteps);
 

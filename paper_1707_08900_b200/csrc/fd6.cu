@@ -980,3 +980,146 @@ extern "C" int fd_debug_poison_ghosts(fd_ctx* c) {
     FD_CHECK_CTX(c);
     return FD_DISPATCH(c, do_poison<T>(c, true));
 }
+
+// ------------------------------------------------------------------------------------------------
+// fd_rhs_static (include/fd6.h): fd_rhs on FD_PATH_55 for callers that cannot allocate device memory.
+//
+// The stencil kernel needs one thing beyond its inputs and outputs: the ghost-padded copy of the four fields it reads
+// (DESIGN.md "HBM layout").  A context gets that from cudaMalloc or the allocator hook; here it is a fixed array in the
+// library image, so the call allocates nothing.  Every GPU that loads libfd6.so holds these bytes until the process ends.
+//
+// `g_static_scratch` below is a device symbol.  In HOST code that name is only a handle the CUDA runtime uses to find the
+// symbol — it is not a device address and must never be handed to a kernel.  The address that kernels can use comes
+// from cudaGetSymbolAddress, asked for once per device with that device current (static_scratch_of_current_device),
+// and it is that pointer which the launches below receive.  All of this has to live in this one .cu file: the array has
+// internal linkage, another translation unit would be looking at a different symbol.
+// ------------------------------------------------------------------------------------------------
+#include <mutex>
+
+static __device__ __align__(256) unsigned char g_static_scratch[FD_RHS_STATIC_MAX_BYTES];
+
+static const int kStaticMaxDevices = 64;
+static std::mutex g_static_mutex;
+static void* g_static_addr[kStaticMaxDevices] = {};  // device address of g_static_scratch on device d; NULL: not asked yet
+
+static int static_scratch_of_current_device(void** out) {
+    int dev = -1;
+    FD_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(FD_EUNSUPPORTED, "fd_rhs_static: device ordinal %d is outside 0..%d", dev, kStaticMaxDevices - 1);
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        FD_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p) return fail(FD_ECUDA, "fd_rhs_static: cudaGetSymbolAddress gave a NULL address on device %d", dev);
+        g_static_addr[dev] = p;
+    }
+    *out = g_static_addr[dev];
+    return FD_OK;
+}
+
+// k_direct_main<T, true> with the update of Eq. 10 taken out: the right-hand side of one cell goes straight to the
+// caller's four dense result arrays (a context's fd_rhs writes it to w first and copies).  Fin is the padded scratch.
+// block (64,4,1), grid (ceil(nx/64), ceil(ny/4), nz), T = float or double (plain layout).
+template <class T>
+__global__ void __launch_bounds__(256) k_rhs55_static(const T* __restrict__ Fin, T* __restrict__ r0, T* __restrict__ r1,
+                                                      T* __restrict__ r2, T* __restrict__ r3, Geom g, Coef<T> c) {
+    const int i = blockIdx.x * 64 + threadIdx.x, j = blockIdx.y * 4 + threadIdx.y, k = blockIdx.z;
+    if (i >= g.nx || j >= g.ny) return;
+    const long long sx = 1, sy = g.px, sz = (long long)g.px * g.py;
+    const long long p = (i + g.gx) + sy * (j + g.gy) + sz * (k + g.gz);
+    const T* l = Fin + p;
+    const T* uu[3] = {Fin + g.fs + p, Fin + 2 * g.fs + p, Fin + 3 * g.fs + p};
+    const long long st[3] = {sx, sy, sz};
+    T u[3], gl[3], G[3][3], L[3], Q[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) gl[a] = d1(l, st[a], c);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        u[q] = uu[q][0];
+        T dd[3];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            G[q][a] = d1(uu[q], st[a], c);
+            dd[a] = d2(uu[q], st[a], c);
+        }
+        L[q] = dd[0] + dd[1] + dd[2];
+        Q[q] = dd[q];
+    }
+    Q[0] += dmix(uu[1], sx, sy, c) + dmix(uu[2], sx, sz, c);
+    Q[1] += dmix(uu[0], sy, sx, c) + dmix(uu[2], sy, sz, c);
+    Q[2] += dmix(uu[0], sz, sx, c) + dmix(uu[1], sz, sy, c);
+    T Rv[4];
+    assemble<T, true>(u, gl, G, L, Q, c, Rv);
+    const long long pw = i + (long long)g.nx * (j + (long long)g.ny * k);
+    r0[pw] = Rv[0];
+    r1[pw] = Rv[1];
+    r2[pw] = Rv[2];
+    r3[pw] = Rv[3];
+}
+
+template <class T>
+static int do_rhs_static(fd_ctx* rec, void* scratch, const void* const in[4], void* const out[4]) {
+    // copy-in + periodic halo fill into the scratch: the helpers a context uses, pointed at the built-in array
+    rec->F[0] = scratch;
+    rec->cur = 0;
+    const T* src[4] = {(const T*)in[0], (const T*)in[1], (const T*)in[2], (const T*)in[3]};
+    int rc = do_pack<T>(rec, src);
+    if (rc) return rc;
+    const Geom& g = rec->g;
+    dim3 block(64, 4, 1), grid((g.nx + 63) / 64, (g.ny + 3) / 4, g.nz);
+    k_rhs55_static<T><<<grid, block, 0, rec->stream>>>((const T*)scratch, (T*)out[0], (T*)out[1], (T*)out[2], (T*)out[3], g,
+                                                       make_coef<T>(rec));
+    FD_CUDA(cudaGetLastError());
+    return FD_OK;
+}
+
+extern "C" int fd_rhs_static(int nx, int ny, int nz, double dx, double nu, double cs, int dtype, const void* lnrho, const void* ux,
+                             const void* uy, const void* uz, void* d_lnrho, void* d_ux, void* d_uy, void* d_uz, void* cuda_stream) {
+    if (!lnrho || !ux || !uy || !uz || !d_lnrho || !d_ux || !d_uy || !d_uz) return fail(FD_EINVAL, "fd_rhs_static: NULL field pointer");
+    if (nx < 8 || ny < 8 || nz < 8) return fail(FD_EINVAL, "fd_rhs_static: every axis needs n >= 8 (got %d,%d,%d)", nx, ny, nz);
+    if (!(dx > 0) || !std::isfinite(dx)) return fail(FD_EINVAL, "fd_rhs_static: dx must be finite and > 0");
+    if (!(nu >= 0) || !std::isfinite(nu)) return fail(FD_EINVAL, "fd_rhs_static: nu must be finite and >= 0");
+    if (!(cs >= 0) || !std::isfinite(cs)) return fail(FD_EINVAL, "fd_rhs_static: cs must be finite and >= 0");
+    if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_rhs_static: bad dtype %d", dtype);
+    if (nx % 4 != 0) return fail(FD_EUNSUPPORTED, "fd_rhs_static: nx must be a multiple of 4 (got %d)", nx);
+    const size_t esize = dtype == FD_F32 ? 4 : 8;
+    // 64-bit size check before make_geom: three axes of >= 8 values each bound every axis by the array size
+    const unsigned long long rough = (unsigned long long)(nx + 8) * (unsigned long long)(ny + 6) * (unsigned long long)(nz + 6) * 4ULL * esize;
+    if (rough > FD_RHS_STATIC_MAX_BYTES)
+        return fail(FD_EUNSUPPORTED,
+                    "fd_rhs_static: the ghost-padded state of a %dx%dx%d %s grid needs at least %llu bytes, the built-in scratch "
+                    "array holds %u (e.g. 64^3 fp32, 48^3 fp64); use fd_create + fd_rhs for larger grids",
+                    nx, ny, nz, dtype == FD_F32 ? "fp32" : "fp64", rough, (unsigned)FD_RHS_STATIC_MAX_BYTES);
+    // A context record on the host stack: only the argument block of the launch helpers (geometry, constants, stream).
+    // It owns no device memory and nothing is allocated for it.
+    fd_ctx rec;
+    rec.nx = nx;
+    rec.ny = ny;
+    rec.nz = nz;
+    rec.dx = dx;
+    rec.nu = nu;
+    rec.cs = cs;
+    rec.dtype = dtype;
+    rec.esize = esize;
+    rec.paired = false;
+    rec.stream = (cudaStream_t)cuda_stream;
+    rec.g = make_geom(nx, ny, nz, esize, false);
+    const unsigned long long need = (unsigned long long)rec.g.fs * 4ULL * esize;
+    if (need > FD_RHS_STATIC_MAX_BYTES)
+        return fail(FD_EUNSUPPORTED,
+                    "fd_rhs_static: the ghost-padded state of a %dx%dx%d %s grid needs %llu bytes, the built-in scratch array "
+                    "holds %u (e.g. 64^3 fp32, 48^3 fp64); use fd_create + fd_rhs for larger grids",
+                    nx, ny, nz, dtype == FD_F32 ? "fp32" : "fp64", need, (unsigned)FD_RHS_STATIC_MAX_BYTES);
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(FD_ECUDA, "fd_rhs_static: no CUDA device (%s); libfd6 has no CPU fallback", cudaGetErrorString(e));
+    }
+    void* scratch = nullptr;
+    int rc = static_scratch_of_current_device(&scratch);
+    if (rc) return rc;
+    const void* in[4] = {lnrho, ux, uy, uz};
+    void* out[4] = {d_lnrho, d_ux, d_uy, d_uz};
+    return dtype == FD_F64 ? do_rhs_static<double>(&rec, scratch, in, out) : do_rhs_static<float>(&rec, scratch, in, out);
+}

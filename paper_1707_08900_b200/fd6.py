@@ -25,7 +25,7 @@ EXPORTS = [
     "fd_set_allocator", "fd_create", "fd_set_path", "fd_set_variant", "fd_set_stream", "fd_load", "fd_store",
     "fd_rhs", "fd_rk3_step", "fd_sync", "fd_destroy", "fd_last_error", "fd_get_info", "fd_kernel_launches",
     "fd_set_profiling", "fd_get_profile", "fd_reset_profile",
-    "fd_plan_work_list", "fd_set_forcing", "fd_set_graphs", "fd_set_tile_shape",
+    "fd_plan_work_list", "fd_set_forcing", "fd_set_graphs", "fd_set_tile_shape", "fd_rhs_static",
 ]
 
 if not os.path.exists(_LIB_PATH):
@@ -74,6 +74,8 @@ lib.fd_set_graphs.argtypes = [_vp, _i]
 lib.fd_set_tile_shape.argtypes = [_vp, _i]
 lib.fd_set_forcing.argtypes = [_vp, C.POINTER(_d), C.POINTER(_d), _d, _d, _d]
 lib.fd_plan_work_list.argtypes = [_i, _i, _i, _i, _i, C.POINTER(FdWorkList)]
+lib.fd_rhs_static.argtypes = [_i, _i, _i, _d, _d, _d, _i] + [_vp] * 9
+FD_RHS_STATIC_MAX_BYTES = 8 * 1024 * 1024
 
 
 def fd_plan_work_list(nx, ny, nz, dtype, sm_count):
@@ -134,6 +136,19 @@ def _ptr(a, where):
     assert a.is_contiguous()
     assert (a.device.type == "cuda") == (where == FD_DEVICE)
     return a.data_ptr()
+
+
+def fd_rhs_static(nx, ny, nz, dx, nu, cs, dtype, state, out):
+    """fd_rhs_static of include/fd6.h: the 55-point right-hand side for callers that cannot allocate device memory
+    (a plug-in inside an application that owns all of the GPU's memory, a loop that must stay clear of cudaMalloc's
+    device-wide synchronisation).  No context, no allocation: the padded copy of the state lives in an 8 MiB array
+    built into libfd6.so, which limits the grid (about 64^3 fp32 / 48^3 fp64) and is shared by all calls on a device,
+    so calls that could overlap on the GPU must be ordered by the caller.  `state` and `out` are four dense CUDA
+    tensors each (or device addresses) on the current device; the work is enqueued on torch's current stream."""
+    import torch
+    ptrs = [_ptr(a, FD_DEVICE) for a in tuple(state) + tuple(out)]
+    _check(lib.fd_rhs_static(int(nx), int(ny), int(nz), float(dx), float(nu), float(cs), int(dtype), *ptrs,
+                             torch.cuda.current_stream().cuda_stream))
 
 
 class Fd:

@@ -97,6 +97,28 @@ def test_argument_validation_happens_before_any_cuda_call(fd6):
     assert L.fd_set_forcing(None, None, None, 0.0, 0.0, 1.0) == fd6.FD_EINVAL
 
 
+def test_fd_rhs_static_validates_before_any_cuda_call(fd6):
+    """The no-allocation entry point checks pointers, parameters and the size limit of its built-in array first."""
+    L = fd6.lib
+    p = C.c_void_p(256)  # never dereferenced: every call below fails on its arguments
+    ok = [p] * 8
+    assert L.fd_rhs_static(32, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32, None, p, p, p, p, p, p, p, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(32, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32, p, p, p, p, p, p, p, None, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(32, 4, 32, 0.1, 0.0, 1.0, fd6.FD_F32, *ok, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(32, 32, 32, -0.1, 0.0, 1.0, fd6.FD_F32, *ok, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(32, 32, 32, 0.1, float("nan"), 1.0, fd6.FD_F32, *ok, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(32, 32, 32, 0.1, 0.0, 1.0, 2, *ok, None) == fd6.FD_EINVAL
+    assert L.fd_rhs_static(30, 32, 32, 0.1, 0.0, 1.0, fd6.FD_F32, *ok, None) == fd6.FD_EUNSUPPORTED
+    # the limit: 64^3 fp32 and 48^3 fp64 fit the 8 MiB array (run on the GPU in tests/test_zz_no_alloc.py); these do not
+    for shape, dtype in (((64, 64, 64), fd6.FD_F64), ((128, 128, 128), fd6.FD_F32), ((2**30, 2**30, 2**30), fd6.FD_F32)):
+        assert L.fd_rhs_static(*shape, 0.1, 0.0, 1.0, dtype, *ok, None) == fd6.FD_EUNSUPPORTED
+        msg = L.fd_last_error().decode()
+        assert "built-in scratch" in msg and str(fd6.FD_RHS_STATIC_MAX_BYTES) in msg
+    header = open(os.path.join(ROOT, "include", "fd6.h")).read()
+    assert re.search(r"#define\s+FD_RHS_STATIC_MAX_BYTES\s+\(8u \* 1024u \* 1024u\)", header)
+    assert fd6.FD_RHS_STATIC_MAX_BYTES == 8 * 1024 * 1024
+
+
 def test_no_cpu_fallback_without_a_device(fd6):
     import torch
     if torch.cuda.is_available():
