@@ -157,10 +157,11 @@ int fd_rhs_static(int nx, int ny, int nz, double dx, double nu, double cs, int d
 /* Advance nsteps full RK3 steps (3 substeps each) of size dt.  FD_EINVAL: nsteps < 0 or dt not finite. */
 int fd_rk3_step(fd_ctx* ctx, double dt, int nsteps);
 
-/* fd_rk3_step enqueues each step as ONE CUDA graph launch (captured on first use, re-captured when dt, the path, the
- * variant or the forcing changes) instead of its 6 (FD_PATH_55) or 15 (FD_PATH_19) kernel launches: the launch rate
- * is what bounds small grids (BASELINE configs C1, C2).  on = 0 switches to plain launches; results are identical.
- * With profiling on (fd_set_profiling) plain launches are used regardless.  Default: on. */
+/* fd_rk3_step enqueues each step as ONE CUDA graph launch instead of its 6 (FD_PATH_55) or 15 (FD_PATH_19) kernel
+ * launches: the launch rate is what bounds small grids (BASELINE configs C1, C2).  The graph is captured once dt, the
+ * path, the variant and the forcing have been the same for 2 consecutive steps (those 2 steps run as plain launches) and
+ * dropped when one of them changes; fd_get_info().graph_state tells which regime is active.  on = 0 switches to plain
+ * launches; results are identical.  With profiling on (fd_set_profiling) plain launches are used regardless.  Default: on. */
 int fd_set_graphs(fd_ctx* ctx, int on);
 
 /* Block until everything enqueued by this context has finished; returns FD_ECUDA if a kernel faulted. */
@@ -180,12 +181,31 @@ typedef struct fd_info {
     int ghost_x, ghost_y, ghost_z;        /* offset of cell (0,0,0) inside a padded array */
     size_t field_stride;                  /* elements between consecutive padded fields   */
     size_t device_bytes;                  /* device memory owned by the context           */
+    /* what fd_rk3_step launches right now (appended fields; the ones above keep their offsets) */
+    int tile_shape;                       /* staged kernels (TILED / PAIRED): 0 wide, 1 tall; -1: the direct kernels run   */
+    int tile_x, tile_y;                   /* tile extents in stored values (0 for the direct kernels)                      */
+    int work_items;                       /* launch grid of the staged main kernel = items of its work list (0: direct)    */
+    int graph_state;                      /* FD_GRAPH_* below                                                               */
+    char graph_note[160];                 /* FD_GRAPH_FAILED: why the capture failed ("" otherwise)                         */
 } fd_info;
+/* graph_state: how the NEXT fd_rk3_step with the same dt would be enqueued.  A step is captured into a CUDA graph only
+ * after dt and every setting a step depends on have stayed the same for 2 consecutive steps, so that a driver which
+ * changes dt or calls fd_set_forcing every step runs plain launches and never pays for a capture. */
+enum {
+    FD_GRAPH_OFF = 0,      /* fd_set_graphs(0): plain launches                                                   */
+    FD_GRAPH_WAITING = 1,  /* on, parameters not yet stable for 2 steps (or profiling on): plain launches         */
+    FD_GRAPH_CAPTURED = 2, /* one graph launch per step                                                          */
+    FD_GRAPH_FAILED = 3    /* capture or instantiation failed for the current parameters: plain launches, not
+                              retried until dt or a setting changes; fd_rk3_step still returns FD_OK              */
+};
 int fd_get_info(const fd_ctx* ctx, fd_info* out);
 
-/* Work list of the tiled kernels (host arithmetic only, needs no CUDA device): the grid is cut
+/* Work list of the STAGED kernels only (FD_VARIANT_TILED / FD_VARIANT_PAIRED; host arithmetic only,
+ * needs no CUDA device).  It is a planning aid: it does not say which variant FD_VARIANT_AUTO resolves to (small grids
+ * run the one-thread-per-cell kernels, which have no work list) nor which shape fd_set_tile_shape forced — for what a
+ * context really launches read fd_get_info (variant, tile_shape, tile_x, tile_y, work_items).  The grid is cut
  * into tiles_x * tiles_y columns of tile_x * tile_y values and `planes` stored planes (nz, or nz/2 in the paired
- * fp32 layout that FD_VARIANT_AUTO picks for even nz).  Item b of the 1-D launch grid is, for b < full_tiles, tile b
+ * fp32 layout, which is planned for fp32 with an even nz >= 8).  Item b of the 1-D launch grid is, for b < full_tiles, tile b
  * over all planes; otherwise, with j = b - full_tiles, tile full_tiles + j / chunks over planes
  * [(j % chunks) * chunk_planes, min(that + chunk_planes, planes)).  Every (tile, plane) is covered exactly once.
  * FD_EINVAL: out == NULL, n < 8, sm_count < 1, bad dtype. */

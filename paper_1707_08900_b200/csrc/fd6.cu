@@ -102,7 +102,15 @@ struct fd_ctx {
     double graph_dt = 0;
     unsigned long long epoch = 0, graph_epoch = ~0ULL;  // epoch: bumped by every setter that changes what a step launches
     cudaStream_t cap_stream = nullptr;
+    // A graph is captured only once (dt, epoch) have held for kGraphAfterSteps consecutive steps: a driver that changes dt or
+    // the forcing every step (PAPER.md:460 draws a new forcing wavevector each step) would otherwise pay a capture and an
+    // instantiation per step, which on small grids costs more than the plain launches the graph replaces.
+    int stable_steps = 0;       // steps run with plain launches under (graph_dt, graph_epoch)
+    bool graph_failed = false;  // capture or instantiation failed under (graph_dt, graph_epoch): plain launches, no retry
+    char graph_note[160] = "";  // why, for fd_get_info
 };
+
+static const int kGraphAfterSteps = 2;
 
 static int ctx_alloc(fd_ctx* c, void** p, size_t bytes) {
     *p = nullptr;
@@ -412,13 +420,34 @@ static int do_rk3(fd_ctx* c, double dt, int nsteps) {
     // the launch rate.  Per-launch profiling needs the individual launches.
     if (c->graphs_on && !c->profiling && nsteps > 0) {
         if (c->graph_epoch != c->epoch || c->graph_dt != dt) {
-            drop_graphs(c);
+            drop_graphs(c);  // nothing to destroy unless the previous parameters had lasted long enough to be captured
             c->graph_epoch = c->epoch;
             c->graph_dt = dt;
+            c->stable_steps = 0;
+            c->graph_failed = false;
+            c->graph_note[0] = 0;
         }
-        for (; n < nsteps; ++n) {
+        for (; n < nsteps && !c->graph_failed; ++n) {
+            if (c->stable_steps < kGraphAfterSteps) {  // parameters not settled yet: plain launches, no capture cost
+                int rc = one_step<T>(c, dt);
+                if (rc) return rc;
+                c->stable_steps++;
+                continue;
+            }
             StepGraph& g = c->graph[c->cur];
-            if (!g.exec && build_graph<T>(c, dt, c->cur) != FD_OK) break;  // plain launches take over
+            if (!g.exec) {
+                char keep[sizeof(g_err)];
+                memcpy(keep, g_err, sizeof(keep));
+                if (build_graph<T>(c, dt, c->cur) != FD_OK) {
+                    // plain launches take over for as long as these parameters last (no retry per call); the failure is kept
+                    // in the context (fd_get_info: graph_state, graph_note), and since this call still succeeds it
+                    // does not leave a message in fd_last_error
+                    c->graph_failed = true;
+                    snprintf(c->graph_note, sizeof(c->graph_note), "%s", g_err);
+                    memcpy(g_err, keep, sizeof(keep));
+                    break;
+                }
+            }
             FD_CUDA(cudaGraphLaunch(g.exec, c->stream));
             c->launches += g.launches;
             c->cur = 1 - c->cur;  // three pointer swaps
@@ -567,6 +596,9 @@ static int set_layout(fd_ctx* c, bool paired) {
 // tensor-map setup fails afterwards the previous layout and variant are restored (c->variant, c->paired and
 // c->tiled always describe the same kernels).
 static int resolve_variant(fd_ctx* c) {
+    // Whatever happens below (also on the failure paths, which may have converted the layout or re-made the tensor maps
+    // before giving up), a step captured earlier no longer describes what a step launches.
+    c->epoch++;
     int want = c->variant_req;
     const bool is_auto = want == FD_VARIANT_AUTO;
     if (is_auto) {
@@ -576,6 +608,9 @@ static int resolve_variant(fd_ctx* c) {
         const long long cells = (long long)c->nx * c->ny * c->nz;
         const bool tiny = cells <= (c->dtype == FD_F64 ? 131072LL : 327680LL);
         want = tiny ? FD_VARIANT_DIRECT : pair_ok(c) ? FD_VARIANT_PAIRED : FD_VARIANT_TILED;
+        if (tiny)
+            snprintf(c->tiled.err, sizeof(c->tiled.err), "automatic variant: grids of at most %lld cells run the one-thread-per-cell kernels",
+                     c->dtype == FD_F64 ? 131072LL : 327680LL);
     }
     if (want == FD_VARIANT_PAIRED && !pair_ok(c))
         return fail(FD_EUNSUPPORTED, "paired variant needs fp32 and an even nz >= 8 (got dtype %d, nz %d)", c->dtype, c->nz);
@@ -587,6 +622,7 @@ static int resolve_variant(fd_ctx* c) {
                 return fail(FD_EUNSUPPORTED,
                             "tiled variant cannot run this grid in the %s layout: it needs >= 4 values per axis and "
                             "4 * padded field size < 2^32 values (the kernels use 32-bit store offsets)", tp ? "paired" : "plain");
+            snprintf(c->tiled.err, sizeof(c->tiled.err), "automatic variant: the staged kernels need >= 4 values per axis and 4 * padded field size < 2^32 values");
             want = FD_VARIANT_DIRECT;
         }
     }
@@ -611,7 +647,6 @@ static int resolve_variant(fd_ctx* c) {
         }
     }
     c->variant = want;
-    c->epoch++;
     return FD_OK;
 }
 
@@ -737,9 +772,17 @@ extern "C" int fd_set_tile_shape(fd_ctx* c, int shape) {
     if (shape < -1 || shape > 1) return fail(FD_EINVAL, "fd_set_tile_shape: shape must be -1 (automatic), 0 (wide) or 1 (tall)");
     const int old = c->tiled.shape_req;
     c->tiled.shape_req = shape;
-    const int rc = resolve_variant(c);
-    if (rc) c->tiled.shape_req = old;
-    return rc;  // re-prepares the tensor maps and the work list of the current variant
+    const int rc = resolve_variant(c);  // re-prepares the tensor maps and the work list of the current variant
+    if (rc) {
+        // the rollback inside resolve_variant still saw the rejected request: put the old one back, then prepare again,
+        // so that shape_req and the prepared launches agree (the message of the refusal is kept)
+        char keep[sizeof(g_err)];
+        memcpy(keep, g_err, sizeof(keep));
+        c->tiled.shape_req = old;
+        resolve_variant(c);
+        memcpy(g_err, keep, sizeof(keep));
+    }
+    return rc;
 }
 
 extern "C" int fd_set_forcing(fd_ctx* c, const double* k, const double* e, double phi, double f0, double dt_ref) {
@@ -870,6 +913,24 @@ extern "C" int fd_get_info(const fd_ctx* c, fd_info* o) {
     o->ghost_z = g.gz;
     o->field_stride = (size_t)g.fs;
     o->device_bytes = c->bytes;
+    const bool staged = c->variant == FD_VARIANT_TILED || c->variant == FD_VARIANT_PAIRED;
+    o->tile_shape = staged ? c->tiled.shape : -1;
+    o->tile_x = o->tile_y = o->work_items = 0;
+    if (staged) {
+        if (c->dtype == FD_F64)
+            shape_dims<double>(c->tiled.shape, &o->tile_x, &o->tile_y);
+        else if (c->paired)
+            shape_dims<V2>(c->tiled.shape, &o->tile_x, &o->tile_y);
+        else
+            shape_dims<float>(c->tiled.shape, &o->tile_x, &o->tile_y);
+        o->work_items = c->tiled.items;
+    }
+    o->graph_state = !c->graphs_on ? FD_GRAPH_OFF
+                     : c->graph_failed ? FD_GRAPH_FAILED
+                     : c->profiling ? FD_GRAPH_WAITING
+                     : (c->graph_epoch == c->epoch && (c->graph[0].exec || c->graph[1].exec)) ? FD_GRAPH_CAPTURED
+                                                                                              : FD_GRAPH_WAITING;
+    snprintf(o->graph_note, sizeof(o->graph_note), "%s", c->graph_note);
     return FD_OK;
 }
 
@@ -911,7 +972,7 @@ extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count
     if (!o) return fail(FD_EINVAL, "fd_plan_work_list: out is NULL");
     if (nx < 8 || ny < 8 || nz < 8 || sm_count < 1) return fail(FD_EINVAL, "fd_plan_work_list: bad grid or SM count");
     if (dtype != FD_F32 && dtype != FD_F64) return fail(FD_EINVAL, "fd_plan_work_list: bad dtype %d", dtype);
-    const bool paired = dtype == FD_F32 && nz % 2 == 0 && nz / 2 >= 4;  // what FD_VARIANT_AUTO resolves to
+    const bool paired = dtype == FD_F32 && nz % 2 == 0 && nz / 2 >= 4;  // the layout the staged kernels would use
     int tx, ty;  // the tile shape tiled_prepare would pick for this grid
     if (dtype == FD_F64)
         shape_dims<double>(pick_shape<double>(nx, ny, sm_count, -1), &tx, &ty);
@@ -970,8 +1031,11 @@ extern "C" int fd_debug_set_tile_overlap(fd_ctx* c, int overlap) {
         rc = fail(FD_EUNSUPPORTED, "fd_debug_set_tile_overlap: the staged kernels do not run this grid with overlap %d (%s)", overlap,
                   tiled_error_of(c->tiled));
     if (rc) {
+        char keep[sizeof(g_err)];
+        memcpy(keep, g_err, sizeof(keep));
         c->tiled.overlap = old;
         resolve_variant(c);
+        memcpy(g_err, keep, sizeof(keep));
     }
     return rc;
 }

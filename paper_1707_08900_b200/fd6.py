@@ -18,6 +18,7 @@ FD_PATH_55, FD_PATH_19 = 0, 1
 FD_HOST, FD_DEVICE = 0, 1
 FD_OK, FD_EINVAL, FD_ENOMEM, FD_ECUDA, FD_EUNSUPPORTED = 0, 1, 2, 3, 4
 FD_VARIANT_AUTO, FD_VARIANT_DIRECT, FD_VARIANT_TILED, FD_VARIANT_PAIRED = 0, 1, 2, 3
+FD_GRAPH_OFF, FD_GRAPH_WAITING, FD_GRAPH_CAPTURED, FD_GRAPH_FAILED = 0, 1, 2, 3
 FD_K_PACK, FD_K_UNPACK, FD_K_HALO, FD_K_FUSED55, FD_K_PASS1, FD_K_PASS2, FD_K_COUNT = range(7)
 KERNEL_NAMES = ["pack", "unpack", "halo", "fused55", "pass1_19", "pass2_19"]
 
@@ -40,7 +41,9 @@ class FdInfo(C.Structure):
     _fields_ = [("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("dtype", C.c_int), ("path", C.c_int),
                 ("variant", C.c_int), ("pitch_x", C.c_int), ("pitch_y", C.c_int), ("pitch_z", C.c_int),
                 ("ghost_x", C.c_int), ("ghost_y", C.c_int), ("ghost_z", C.c_int),
-                ("field_stride", C.c_size_t), ("device_bytes", C.c_size_t)]
+                ("field_stride", C.c_size_t), ("device_bytes", C.c_size_t),
+                ("tile_shape", C.c_int), ("tile_x", C.c_int), ("tile_y", C.c_int), ("work_items", C.c_int),
+                ("graph_state", C.c_int), ("graph_note", C.c_char * 160)]
 
 
 class FdWorkList(C.Structure):

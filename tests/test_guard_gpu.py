@@ -81,7 +81,7 @@ def test_no_write_outside_allocations(shape, dtype):
                 for graphs in (True, False):
                     ctx.fd_set_graphs(graphs)
                     ctx.load_state(F)
-                    ctx.fd_rk3_step(0.02, 1)
+                    ctx.fd_rk3_step(0.02, 3)  # with graphs on: two plain steps, then one captured step
                     ctx.rhs_state()
                     ctx.store_state()
                     ran += 1

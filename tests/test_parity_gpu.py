@@ -418,7 +418,8 @@ def test_many_tiles_few_planes(mods, shape, dtype, path):
 def test_graph_steps_equal_plain_launches_bitwise(mods, dtype, shape, path):
     """One graph launch per step must enqueue exactly the launches of the plain path: same bits and the same launch
     count, across an odd number of steps (the read copy alternates), a change of dt, of the forcing and of the variant
-    (each re-captures), and with the oracle as the referee of the whole trajectory."""
+    (each drops the graphs; a new one is captured once the new parameters have held for two steps), and with the oracle
+    as the referee of the whole trajectory."""
     O, fd6, I = mods
     rng = np.random.default_rng(77 + path)
     dx, nu, cs = 0.2, 0.02, 1.0
@@ -430,19 +431,26 @@ def test_graph_steps_equal_plain_launches_bitwise(mods, dtype, shape, path):
         ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32 if dtype == "f32" else fd6.FD_F64)
         ctx.fd_set_path(path)
         ctx.fd_set_graphs(graphs)
+        captured = fd6.FD_GRAPH_CAPTURED if graphs else fd6.FD_GRAPH_OFF
+        waiting = fd6.FD_GRAPH_WAITING if graphs else fd6.FD_GRAPH_OFF
         ctx.load_state(F)
         n0 = ctx.fd_kernel_launches()
-        ctx.fd_rk3_step(dt, 3)
-        ctx.fd_rk3_step(dt, 2)
+        ctx.fd_rk3_step(dt, 3)  # two plain steps while the parameters settle, then the first captured step
+        assert ctx.fd_get_info().graph_state == captured
+        ctx.fd_rk3_step(dt, 2)  # the graph of the other read copy, then the first one again
         a = ctx.store_state()
         ctx.fd_rk3_step(0.5 * dt, 1)
+        assert ctx.fd_get_info().graph_state == waiting  # a new dt: plain launches, nothing captured for one step
         ctx.fd_set_forcing(kf, ef, 0.3, 0.02, dt)
-        ctx.fd_rk3_step(dt, 2)
+        ctx.fd_rk3_step(dt, 4)  # forced steps: two plain, then one graph per read copy
+        assert ctx.fd_get_info().graph_state == captured
         ctx.fd_set_forcing(None, None, 0.0, 0.0, dt)
         ctx.fd_set_variant(fd6.FD_VARIANT_DIRECT)
-        ctx.fd_rk3_step(dt, 1)
+        ctx.fd_rk3_step(dt, 3)
+        assert ctx.fd_get_info().graph_state == captured
         b = ctx.store_state()
         n = ctx.fd_kernel_launches() - n0
+        assert ctx.fd_get_info().graph_note == b""
         ctx.fd_destroy()
         return a, b, n
 
@@ -453,6 +461,38 @@ def test_graph_steps_equal_plain_launches_bitwise(mods, dtype, shape, path):
     assert all(np.array_equal(x, y) for x, y in zip(b1, b0))
     ref = O.rk3_step(F.astype(np.float64), dx, nu, cs, dt, 5, path)
     assert relinf(a1, ref) <= 5 * TOL[dtype]
+
+
+def test_parameters_that_change_every_step_never_pay_for_a_capture(mods):
+    """A driver that draws a new forcing wavevector every step or adapts dt every step must run plain
+    launches (graph_state stays FD_GRAPH_WAITING: no capture, no instantiation per step) with the bits of graphs-off."""
+    O, fd6, I = mods
+    shape, dx, nu, cs = (40, 26, 24), 0.2, 0.02, 1.0
+    dt = 0.1 * dx
+    F = smooth_state(np.random.default_rng(5), shape, 0.1, "f32")
+    k1 = TWO_PI / (shape[0] * dx)
+
+    def run(graphs):
+        ctx = fd6.Fd(*shape, dx, nu, cs, fd6.FD_F32)
+        ctx.fd_set_graphs(graphs)
+        ctx.load_state(F)
+        states = []
+        for s in range(6):
+            ctx.fd_set_forcing((k1 * (1 + s % 3), 0.0, 0.0), (0.0, 1.0, 0.0), 0.1 * s, 0.02, dt)
+            ctx.fd_rk3_step(dt, 1)
+            states.append(ctx.fd_get_info().graph_state)
+        for s in range(6):
+            ctx.fd_rk3_step(dt * (1.0 + 0.01 * s), 1)
+            states.append(ctx.fd_get_info().graph_state)
+        out = ctx.store_state()
+        n = ctx.fd_kernel_launches()
+        ctx.fd_destroy()
+        return out, states, n
+
+    g, sg, ng = run(True)
+    p, sp, np_ = run(False)
+    assert sg == [fd6.FD_GRAPH_WAITING] * 12 and sp == [fd6.FD_GRAPH_OFF] * 12
+    assert ng == np_ and all(np.array_equal(x, y) for x, y in zip(g, p))
 
 
 # ------------------------------------------------- BASELINE config C2 as stated: 100 RK3 steps, both stencil paths
