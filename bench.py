@@ -10,7 +10,11 @@ the whole grid.  Workload at N = 1: config C4 of BASELINE.json (512^3 fp32, seed
 N > 1: independent replicas (the north_star path is single-GPU; no collective is
 invented), value = cells of all ranks x K / max-over-ranks device time.
 
-value        device-resident: K steps in one fd_rk3_step(dt, K) call, CUDA events on the launching stream.
+value        device-resident: K steps in one fd_rk3_step(dt, K) call, CUDA events on the launching stream; the call is
+             repeated --reps times (default 5) back to back from the same state and `value` is the MEDIAN repetition
+             (value_min / value_max / values beside it; the clock sampler runs across all repetitions).
+value_sustained  the same call sized to run >= 1.2 s (the board's power cap engages after ~0.1 s of this kernel): the
+             figure that answers "sustains"; details under "sustained".
 e2e          the same job through the C ABI with HOST (pinned) buffers: fd_load(host) + fd_rk3_step(dt, K) +
              fd_store(host), copies inside the timed region; bytes per step = job bytes / K.  The variant
              with a load and a store around EVERY step is reported as e2e.every_step_io.
@@ -229,6 +233,10 @@ def main():
     ap.add_argument("--no-sustained", action="store_true", help="skip the >= 1 s sustained measurement")
     ap.add_argument("--sustained-seconds", type=float, default=1.2)
     ap.add_argument("--cpu-budget", type=float, default=15.0)
+    ap.add_argument("--reps", type=int, default=5, help="repetitions of the timed K-step call; value = their median")
+    ap.add_argument("--forcing-every-step", action="store_true",
+                    help="extra measurement: fd_set_forcing with a new wavevector before every single step (PAPER.md:460), "
+                         "the case in which a step is never captured into a CUDA graph")
     args = ap.parse_args()
 
     from paper_1707_08900_b200 import inputs
@@ -269,11 +277,13 @@ def main():
     if args.tile_overlap:
         from paper_1707_08900_b200 import fd6_testing
         fd6_testing.fd_debug_set_tile_overlap(ctx, args.tile_overlap)
-    info = ctx.fd_get_info()
-    wl = fd6.fd_plan_work_list(n, n, n, fd6.FD_F32 if cfg.dtype == "f32" else fd6.FD_F64, 148)
-    tile = {0: "wide 32x12", 1: "tall 32x16"}.get(args.tile_shape, f"automatic ({wl.tile_x}x{wl.tile_y})") if info.variant in (2, 3) else None
-    if info.variant == 2 and cfg.dtype == "f32":
-        tile = "32x24 cells (y pairs)"
+    info = ctx.fd_get_info()  # what the context really launches (variant, prepared tile shape, work items)
+    tile = None
+    if info.variant in (2, 3):
+        tile = (f"{'automatic' if args.tile_shape < 0 else 'forced'}: {('wide', 'tall')[info.tile_shape]} "
+                f"{info.tile_x}x{info.tile_y} values, {info.work_items} work items")
+        if info.variant == 2 and cfg.dtype == "f32":
+            tile += " (y pairs)"
     forcing = dict(k=(3.0, 2.0, -4.0), e=(0.36, -0.48, 0.8), phi=0.7, f0=0.05) if args.forcing else None
     if forcing:
         ctx.fd_set_forcing(forcing["k"], forcing["e"], forcing["phi"], forcing["f0"], cfg.dt)
@@ -282,45 +292,85 @@ def main():
     stream = torch.cuda.current_stream()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
 
-    def timed_steps(nsteps, profiling):
-        """nsteps steps from the config's state in ONE fd_rk3_step call, CUDA events on the launching stream."""
-        ctx.load_state(F0)
+    def timed_steps(nsteps, profiling, reps=1):
+        """`reps` times: nsteps steps from the config's state in ONE fd_rk3_step call, CUDA events on the launching stream.
+        Returns the per-repetition device times (ms), the launches of one repetition, the clock record, the profile."""
         ctx.fd_set_profiling(profiling)
-        if profiling:
-            ctx.fd_reset_profile()
-        barrier()
-        n0 = ctx.fd_kernel_launches()
+        times, n_launch = [], 0
         with ClockSampler(local) as clk_:
-            e0.record(stream)
-            ctx.fd_rk3_step(cfg.dt, nsteps)
-            e1.record(stream)
-            barrier()
+            for _ in range(reps):
+                ctx.load_state(F0)
+                if profiling:
+                    ctx.fd_reset_profile()
+                barrier()
+                n0 = ctx.fd_kernel_launches()
+                e0.record(stream)
+                ctx.fd_rk3_step(cfg.dt, nsteps)
+                e1.record(stream)
+                barrier()
+                times.append(e0.elapsed_time(e1))
+                n_launch = ctx.fd_kernel_launches() - n0
         prof_ = {fd6.KERNEL_NAMES[k]: ctx.fd_get_profile(k) for k in range(fd6.FD_K_COUNT)} if profiling else None
         ctx.fd_set_profiling(False)
-        return e0.elapsed_time(e1), ctx.fd_kernel_launches() - n0, clk_, prof_
+        return times, n_launch, clk_, prof_
 
-    # pass 1: `value` - right after the W warm-up steps, profiling off, each step one CUDA graph launch
-    ms, launches, clk, _ = timed_steps(K, False)
+    # pass 1: `value` - right after the W warm-up steps, profiling off, each step one CUDA graph launch; the median of
+    # `reps` back-to-back repetitions (SURVEY 8(d): >= 5 repetitions, report median and min)
+    reps = max(1, args.reps)
+    rep_ms, launches, clk, _ = timed_steps(K, False, reps)
+    graph_state = ctx.fd_get_info().graph_state
+    rep_ms = sorted(max_ms(t) for t in rep_ms)
+    ms_max = rep_ms[len(rep_ms) // 2] if len(rep_ms) % 2 else 0.5 * (rep_ms[len(rep_ms) // 2 - 1] + rep_ms[len(rep_ms) // 2])
     # pass 2: the per-kernel profile (two event records around every launch: kept out of `value`)
     prof_ms, _, _, prof = timed_steps(K, True)
+    prof_ms = max_ms(prof_ms[0])
     chk = torch.empty_like(F0)
     ctx.store_state(chk)
     ctx.fd_sync()
     finite = bool(torch.isfinite(chk).all().item())
     del chk
-    ms_max = max_ms(ms)
-    prof_ms = max_ms(prof_ms)
     value = replicas.whole_job_value(N, K, ms_max, world)
+    rep_values = [replicas.whole_job_value(N, K, t, world) for t in rep_ms]  # descending
 
     # pass 3: the same measurement sustained over >= 1 s (the 1 kW power cap engages after ~0.1 s of this kernel)
     sustained = None
     if not args.no_sustained:
         Ks = max(K, int(math.ceil(args.sustained_seconds * 1e3 / (ms_max / K))))
         s_ms, _, s_clk, _ = timed_steps(Ks, False)
-        s_ms = max_ms(s_ms)
+        s_ms = max_ms(s_ms[0])
         sustained = {"value": replicas.whole_job_value(N, Ks, s_ms, world), "unit": UNIT, "steps": Ks, "seconds": s_ms * 1e-3,
                      "ms_per_step": s_ms / Ks, "clocks": s_clk.summary()}
         sustained["vs_burst"] = sustained["value"] / value
+
+    # optional: a new forcing wavevector before EVERY step (PAPER.md:460): fd_set_forcing + fd_rk3_step(dt, 1), K times
+    forcing_each = None
+    if args.forcing_every_step:
+        kf0 = 2 * math.pi / (n * cfg.dx)
+
+        def forced_steps(count):
+            for s_ in range(count):
+                ctx.fd_set_forcing((kf0 * (2 + s_ % 3), kf0 * (1 + s_ % 2), -kf0 * 3), (0.36, -0.48, 0.8), 0.1 * s_, 0.05, cfg.dt)
+                ctx.fd_rk3_step(cfg.dt, 1)
+
+        ctx.load_state(F0)
+        forced_steps(3)
+        fe = []
+        for _ in range(reps):
+            ctx.load_state(F0)
+            barrier()
+            e0.record(stream)
+            forced_steps(K)
+            e1.record(stream)
+            barrier()
+            fe.append(max_ms(e0.elapsed_time(e1)))
+        fe.sort()
+        forcing_each = {"value": replicas.whole_job_value(N, K, fe[len(fe) // 2], world), "unit": UNIT,
+                        "ms_per_step": fe[len(fe) // 2] / K, "graph_state_after": int(ctx.fd_get_info().graph_state),
+                        "note": "fd_set_forcing (host tables, one H2D copy, a stream synchronise) + fd_rk3_step(dt, 1) per step; "
+                                "graph_state 1 = FD_GRAPH_WAITING: plain launches, nothing captured"}
+        ctx.fd_set_forcing(None, None, 0.0, 0.0, cfg.dt)
+        if forcing:
+            ctx.fd_set_forcing(forcing["k"], forcing["e"], forcing["phi"], forcing["f0"], cfg.dt)
 
     state_mb = 4 * N * esize / 1e6
     l2_note = (f"inputs larger than L2 ({state_mb / 1e3:.1f} GB state, {16 * esize * N / 1e9:.1f} GB streamed per substep); no flush needed"
@@ -347,14 +397,14 @@ def main():
     barrier()
     e2e_ms = max_ms(e0.elapsed_time(e1))
     e2e_value = replicas.whole_job_value(N, K, e2e_ms, world)
-    reps = 3
+    io_reps = 3
     barrier()
     e0.record(stream)
-    for _ in range(reps):
+    for _ in range(io_reps):
         e2e_job(1)
     e1.record(stream)
     barrier()
-    e2e_each = replicas.whole_job_value(N, reps, max_ms(e0.elapsed_time(e1)), world)
+    e2e_each = replicas.whole_job_value(N, io_reps, max_ms(e0.elapsed_time(e1)), world)
     finite = finite and bool(torch.isfinite(host_out).all().item())
 
     # ---- roofline of the dominant kernel
@@ -399,7 +449,10 @@ def main():
             "config": {"workload": f"{cfg.name}: {n}^3 periodic {cfg.dtype}, band-limited |k|<={cfg.kmax} rms Mach {cfg.amp}, "
                                    f"nu={cfg.nu}, dt=0.1 dx/cs", "path": f"{args.path}-point",
                        "variant": variant_name, "tile_shape": tile, "tile_overlap": args.tile_overlap,
-                       "l2": l2_note, "launch": "one CUDA graph per RK3 step (fd_set_graphs on)",
+                       "l2": l2_note,
+                       "launch": {0: "plain launches (graphs off)", 1: "plain launches (graph not captured)",
+                                  2: "one CUDA graph per RK3 step (fd_get_info: FD_GRAPH_CAPTURED)",
+                                  3: "plain launches (graph capture failed: " + info.graph_note.decode() + ")"}[int(graph_state)],
                        "parallelism": "replicas only" if world > 1 else "single GPU", "finite": finite,
                        "forcing": (f"on: k={forcing['k']}, f0={forcing['f0']}" if forcing else "off (PAPER.md:369)")},
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": state_bytes / K,
@@ -409,8 +462,15 @@ def main():
                                       "d2h_bytes_per_step": state_bytes}},
             "gpu_launches": int(launches), "clocks": clk.summary(), "roofline": roofline,
         }
+        line["value_min"], line["value_max"] = rep_values[-1], rep_values[0]
+        line["values"] = [round(v, 1) for v in rep_values]
+        line["reps"] = reps
+        line["value_is"] = f"median of {reps} back-to-back repetitions of fd_rk3_step(dt, {K})"
         if sustained is not None:
+            line["value_sustained"] = sustained["value"]
             line["sustained"] = sustained
+        if forcing_each is not None:
+            line["forcing_every_step"] = forcing_each
         if cpu_baseline is not None:
             line["cpu_baseline"] = cpu_baseline
         print(json.dumps(line), flush=True)
