@@ -215,9 +215,9 @@ def test_shear_mode_decay_closed_form_on_gpu(mods, path, variant):
 
 
 # ------------------------------- big grids: windowed oracle on sampled blocks
-def _sample_origins(n, size, rng, extra):
+def _sample_origins(n, size, rng, extra, count=8):
     pts = [(0, 0, 0), (n - size // 2, n - size // 2, n - size // 2), (n - 7, 3, n // 2)] + list(extra)
-    while len(pts) < 8:
+    while len(pts) < count:
         pts.append(tuple(int(v) for v in rng.integers(0, n, 3)))
     return pts
 
@@ -244,7 +244,7 @@ def _windowed_check(mods, cfg_name, path, variant, n_override=None, inner=16, nb
     # blocks at the periodic seam, at the origin, across tile boundaries (multiples of 64/16) and random ones
     extra = [(64 - m - 3, 16 - m - 2, n // 2 - m), (n // 2 - m - 1, n - m - 5, 5)]
     worst = 0.0
-    for origin in _sample_origins(n, size, rng, extra)[:nblocks]:
+    for origin in _sample_origins(n, size, rng, extra, nblocks)[:nblocks]:
         sub = I.gather_block(F, origin, size).astype(np.float64)
         ref, mm = O.rk3_step_window(sub, dx, cfg.nu, cfg.cs, dt, 1, path)
         got = I.gather_block(out, tuple(o + m for o in origin), inner)
@@ -262,8 +262,9 @@ def test_c3_256_fp64_sampled_blocks(mods, path):
 
 @pytest.mark.parametrize("path", [0, 1])
 def test_c4_512_fp32_sampled_blocks_in_the_bench_configuration(mods, path):
-    """Full headline size, default (AUTO) variant = the launch configuration bench.py times."""
-    assert _windowed_check(mods, "C4", path, 0) <= TOL["f32"]
+    """Full headline size, default (AUTO) variant = the launch configuration bench.py times; 16 blocks of 32^3
+     at the periodic seam, the z-pairing seam, tile edges and random places."""
+    assert _windowed_check(mods, "C4", path, 0, inner=32, nblocks=16) <= TOL["f32"]
 
 
 @pytest.mark.parametrize("path", [0, 1])
@@ -283,7 +284,7 @@ def test_c5_1024_fp32_sampled_blocks(mods, path):
         assert e.value.code == fd6.FD_EUNSUPPORTED and "2^32" in str(e.value)
         assert ctx.fd_get_info().variant == fd6.FD_VARIANT_PAIRED
 
-    assert _windowed_check(mods, "C5", path, 0, nblocks=6, before_step=rejected_switch if path == 0 else None) <= TOL["f32"]
+    assert _windowed_check(mods, "C5", path, 0, inner=32, nblocks=16, before_step=rejected_switch if path == 0 else None) <= TOL["f32"]
 
 
 def test_c3_256_fp64_full_grid_55(mods):
@@ -297,6 +298,74 @@ def test_c3_256_fp64_full_grid_55(mods):
     ref = O.rk3_step(F, cfg.dx, cfg.nu, cfg.cs, cfg.dt, 1, 0)
     assert relinf(got, ref) <= TOL["f64"]
     ctx.fd_destroy()
+
+
+# ------------------------------------------------- fd_rhs against the oracle: every kernel that can produce it
+@pytest.mark.parametrize("shape", [(132, 70, 20), (72, 33, 41)])
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("path", [0, 1])
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_fd_rhs_on_ragged_multi_tile_grids(mods, dtype, path, variant, shape):
+    """fd_rhs is one of the six calls north_star names: right-hand side of Eq. 1-3 from the direct kernels (write_f = 0),
+    the staged kernels in update mode 2 (plain fp32 = y pairs, fp64, paired fp32) and, on the 19-point path, pass 1 +
+    pass 2 with write_f = 0, on shapes with several tiles per axis, ragged tails and (41 planes) an odd plane count."""
+    O, fd6, I = mods
+    rng = np.random.default_rng(1000 + 7 * path + variant)
+    dx, nu, cs = 0.1, 0.02, 1.0
+    F = smooth_state(rng, shape, 0.1, dtype)
+    ctx = make_ctx(fd6, shape, dx, nu, cs, dtype, path, variant)
+    ctx.load_state(F)
+    T.fd_debug_poison_w(ctx)  # the w scratch fd_rhs writes through must not be read
+    R = ctx.rhs_state()
+    assert np.array_equal(ctx.store_state(), F)
+    ctx.fd_destroy()
+    assert relinf(R, O.rhs(F.astype(np.float64), dx, nu, cs, path)) <= TOL[dtype]
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3])
+@pytest.mark.parametrize("path", [0, 1])
+def test_fd_rhs_c2_full_grid_fp32(mods, path, variant):
+    O, fd6, I = mods
+    cfg = I.CONFIGS["C2"]
+    F = I.make_state(cfg)
+    ctx = make_ctx(fd6, (cfg.n,) * 3, cfg.dx, cfg.nu, cfg.cs, "f32", path, variant)
+    ctx.load_state(F)
+    R = ctx.rhs_state()
+    ctx.fd_destroy()
+    assert relinf(R, O.rhs(F.astype(np.float64), cfg.dx, cfg.nu, cfg.cs, path)) <= TOL["f32"]
+
+
+@pytest.mark.parametrize("cfg_name,variant", [("C3", 2), ("C4", 0)])
+@pytest.mark.parametrize("path", [0, 1])
+def test_fd_rhs_big_grids_sampled_blocks(mods, cfg_name, variant, path):
+    """fd_rhs on grids with more than one wave of tiles and a z-chunked remainder (C3 fp64 staged kernels, C4 fp32 in the
+    bench configuration).  The right-hand side is local (radius 3; 6 on the 19-point path, whose pass 2 differentiates
+    div u again), so the oracle runs on a periodic sub-block and only the cells further than that from its faces count."""
+    import torch
+    O, fd6, I = mods
+    cfg = I.CONFIGS[cfg_name]
+    n = cfg.n
+    F = I.make_state(cfg, device="cuda")
+    ctx = make_ctx(fd6, (n,) * 3, cfg.dx, cfg.nu, cfg.cs, cfg.dtype, path, variant)
+    ctx.load_state(F)
+    R = torch.empty_like(F)
+    ctx.rhs_state(R)
+    ctx.fd_sync()
+    m = 3 if path == 0 else 6
+    inner = 32
+    size = inner + 2 * m
+    rng = np.random.default_rng(cfg.seed + 17)
+    extra = [(64 - m - 3, 16 - m - 2, n // 2 - m), (n // 2 - m - 1, n - m - 5, 5)]
+    worst = 0.0
+    for origin in _sample_origins(n, size, rng, extra, 16):
+        sub = I.gather_block(F, origin, size).astype(np.float64)
+        ref = O.rhs(sub, cfg.dx, cfg.nu, cfg.cs, path)[:, m:-m, m:-m, m:-m]
+        got = I.gather_block(R, tuple(o + m for o in origin), inner)
+        worst = max(worst, relinf(got, ref))
+    ctx.fd_destroy()
+    del F, R
+    torch.cuda.empty_cache()
+    assert worst <= TOL[cfg.dtype]
 
 
 # ------------------------------------------------------------------------ error behaviour
