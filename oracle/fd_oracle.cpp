@@ -19,6 +19,11 @@
 // (it is pinned only through the per-substep closed form P3, the linear closed
 // form P6 and the 19-vs-55 O(dx^6) agreement).
 //
+// Not reentrant: fdo_set_forcing stores the forcing term in a file-static that every later fdo_rhs_* / fdo_rk3_step_*
+// call of the PROCESS reads, so two threads (or two interleaved users) with different forcings would see each other's;
+// oracle/oracle.py sets and clears it around each call (`with forcing(...)`).  Fine for a test oracle; do not call the
+// fdo_* functions concurrently.
+//
 // Build: oracle/build.py  (g++ -O2 -ffp-contract=off -fopenmp, no -ffast-math).
 // The only parallelism is one `#pragma omp parallel for` over k-planes; every cell
 // is independent inside a sweep, so threading does not change any result bit.
