@@ -267,6 +267,90 @@ __global__ void __launch_bounds__(256) k_direct_pass2_x2(const float* __restrict
     }
 }
 
+// a8 for the staged variants (8-byte value types: fp64 and the paired fp32 layout): two x-adjacent values per thread with
+// 16-byte accesses, marching along z with the seven div planes of the z derivative in a register window, so a value costs
+// 5.5 div loads of 16 bytes instead of 18 of 8 (4 for x beside the window's centre, 6 for y, 1 new plane for z, per pair)
+// and every load of an iteration is issued before the first use.  nx is even (fd_create: nx % 4 == 0), rows of the padded
+// and of the dense arrays start 32-byte aligned, so the pairs (2i, 2i+1) are 16-byte aligned; the x ghost pad holds 4
+// values, which covers the aligned pair at i - 4 (its low half is never used).  Arithmetic per value is the expression of
+// d1() on the same operands: results equal k_direct_pass2 bitwise.  Measured on B200 (profiles/r03_bench_C*_19.json.txt):
+// C4 pass 2 1.19 -> 1.05 ms per launch, C5 +7.5 % per step; chunks of 8, 16 and 32 planes are within 0.3 %, 64 is 1.6 %
+// slower; evict-first (ld/st.global.cs) accesses for w and F_out were 3 % SLOWER per step and are not used.
+// grid = (ceil(nx/128), ceil(ny/4), ceil(nz/zc)), block (64, 4); a thread updates planes [blockIdx.z * zc, + zc).
+template <class T>
+struct __align__(16) Pair2 {
+    T x, y;
+};
+template <class T>
+__device__ __forceinline__ T d1v(T p1, T m1, T p2, T m2, T p3, T m3, const Coef<T>& c) {
+    return c.a1 * (p1 - m1) + c.a2 * (p2 - m2) + c.a3 * (p3 - m3);
+}
+template <class T>
+__global__ void __launch_bounds__(256) k_pass2_march(const T* __restrict__ Div, T* __restrict__ Fout, T* __restrict__ W, Geom g,
+                                                     Coef<T> c, Sub<T> s, int zc) {
+    static_assert(sizeof(T) == 8, "two 8-byte values per 16-byte access");
+    typedef Pair2<T> P;
+    const int i = 2 * (blockIdx.x * 64 + threadIdx.x), j = blockIdx.y * 4 + threadIdx.y, k0 = blockIdx.z * zc;
+    if (i >= g.nx || j >= g.ny) return;
+    const int k1 = min(k0 + zc, g.nz);
+    const long long sy = g.px, sz = (long long)g.px * g.py;
+    const T* d = Div + (i + g.gx) + sy * (j + g.gy) + sz * (k0 + g.gz);
+    T* f = Fout + g.fs + (i + g.gx) + sy * (j + g.gy) + sz * (k0 + g.gz);
+    T* w = W + g.n + i + (long long)g.nx * (j + (long long)g.ny * k0);
+    const long long wz = (long long)g.nx * g.ny;
+    auto ld = [](const T* p) { return *reinterpret_cast<const P*>(p); };
+    auto st = [](T* p, P v) { *reinterpret_cast<P*>(p) = v; };
+    const T scale = s.dt * c.nu3;
+    P zm3 = ld(d - 3 * sz), zm2 = ld(d - 2 * sz), zm1 = ld(d - sz), z0 = ld(d), zp1 = ld(d + sz), zp2 = ld(d + 2 * sz);
+    for (int k = k0; k < k1; ++k) {
+        const P zp3 = ld(d + 3 * sz);
+        const P xa = ld(d - 4), xb = ld(d - 2), xd = ld(d + 2), xe = ld(d + 4);
+        const P yp1 = ld(d + sy), ym1 = ld(d - sy), yp2 = ld(d + 2 * sy), ym2 = ld(d - 2 * sy), yp3 = ld(d + 3 * sy), ym3 = ld(d - 3 * sy);
+        P wv[3], fv[3];
+        if (s.write_w) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) wv[a] = ld(w + a * g.n);
+        }
+        if (s.write_f) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) fv[a] = ld(f + a * g.fs);
+        }
+        P add[3];
+        // Eq. 6 along x for values i and i + 1 from the aligned pairs that cover i-3 .. i+4 (z0 is the pair itself)
+        add[0].x = scale * d1v(z0.y, xb.y, xd.x, xb.x, xd.y, xa.y, c);
+        add[0].y = scale * d1v(xd.x, z0.x, xd.y, xb.y, xe.x, xb.x, c);
+        add[1].x = scale * d1v(yp1.x, ym1.x, yp2.x, ym2.x, yp3.x, ym3.x, c);
+        add[1].y = scale * d1v(yp1.y, ym1.y, yp2.y, ym2.y, yp3.y, ym3.y, c);
+        add[2].x = scale * d1v(zp1.x, zm1.x, zp2.x, zm2.x, zp3.x, zm3.x, c);
+        add[2].y = scale * d1v(zp1.y, zm1.y, zp2.y, zm2.y, zp3.y, zm3.y, c);
+        if (s.write_w) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                wv[a].x += add[a].x;
+                wv[a].y += add[a].y;
+                st(w + a * g.n, wv[a]);
+            }
+        }
+        if (s.write_f) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                fv[a].x += s.beta * add[a].x;
+                fv[a].y += s.beta * add[a].y;
+                st(f + a * g.fs, fv[a]);
+            }
+        }
+        zm3 = zm2;
+        zm2 = zm1;
+        zm1 = z0;
+        z0 = zp1;
+        zp1 = zp2;
+        zp2 = zp3;
+        d += sz;
+        f += sz;
+        w += wz;
+    }
+}
+
 // Test hooks: poison w / all ghost cells with NaN.
 template <class T>
 __global__ void k_fill(T* __restrict__ a, long long n, T v) {
