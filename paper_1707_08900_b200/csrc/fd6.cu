@@ -341,7 +341,10 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
             // z derivative stay in registers, so no y banding is needed to keep them in L2)
             const int zc = 16;  // planes per thread: 6 warm-up div loads per 16 planes, 16 chunk layers at C4
             dim3 grid2((g.nx + 127) / 128, (g.ny + 3) / 4, (g.nz + zc - 1) / zc);
-            k_pass2_march<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s, zc);
+            if (s.write_w)
+                k_pass2_march<T, true><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s, zc);
+            else
+                k_pass2_march<T, false><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s, zc);
         } else {
             dim3 grid2((g.nx + 63) / 64, band_rows, bands * g.nz);
             k_direct_pass2<T><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
