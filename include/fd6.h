@@ -207,11 +207,15 @@ int fd_get_info(const fd_ctx* ctx, fd_info* out);
  * into tiles_x * tiles_y columns of tile_x * tile_y values and `planes` stored planes (nz, or nz/2 in the paired
  * fp32 layout, which is planned for fp32 with an even nz >= 8).  Item b of the 1-D launch grid is, for b < full_tiles, tile b
  * over all planes; otherwise, with j = b - full_tiles, tile full_tiles + j / chunks over planes
- * [(j % chunks) * chunk_planes, min(that + chunk_planes, planes)).  Every (tile, plane) is covered exactly once.
+ * [(j % chunks) * chunk_planes, min(that + chunk_planes, planes)) — unless split_plane > 0, see below.  Every (tile,
+ * plane) is covered exactly once.
  * FD_EINVAL: out == NULL, n < 8, sm_count < 1, bad dtype. */
 typedef struct fd_work_list {
     int tile_x, tile_y, tiles_x, tiles_y, planes;
     int full_tiles, chunks, chunk_planes, items;
+    int split_plane; /* 0, or the split list (grids with about as many tiles as SMs): full_tiles = 0, items = 2 * tiles;
+                        item b < tiles is tile b over planes [0, split_plane), item tiles + b is tile b over
+                        [split_plane, planes): the long parts are dispatched first, the short ones fill the idle SMs */
 } fd_work_list;
 int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count, fd_work_list* out);
 

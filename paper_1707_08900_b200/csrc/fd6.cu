@@ -1000,6 +1000,7 @@ extern "C" int fd_plan_work_list(int nx, int ny, int nz, int dtype, int sm_count
     o->full_tiles = sc.n_full;
     o->chunks = sc.k;
     o->chunk_planes = sc.zc;
+    o->split_plane = sc.za;
     o->items = items;
     return FD_OK;
 }

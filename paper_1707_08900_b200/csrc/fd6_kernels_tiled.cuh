@@ -578,7 +578,15 @@ struct Tiled {
         const int tid = ty * TX + tx;
         const bool lane0 = (tid & 31) == 0, producer = tid == 0;
         int tile = blockIdx.x, zs = 0, ze = g.nz;
-        if (tile >= sc.n_full) {
+        if (sc.za > 0) {  // split list: every tile cut at plane za, the long parts first
+            const int nt = sc.ntx * sc.nty;
+            if (tile >= nt) {
+                tile -= nt;
+                zs = sc.za;
+            } else {
+                ze = sc.za;
+            }
+        } else if (tile >= sc.n_full) {
             const int j = tile - sc.n_full;
             tile = sc.n_full + j / sc.k;
             zs = (j % sc.k) * sc.zc;

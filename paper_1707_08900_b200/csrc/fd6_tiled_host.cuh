@@ -6,7 +6,10 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <functional>
+#include <queue>
 #include <type_traits>
+#include <vector>
 
 #include "fd6_common.cuh"
 
@@ -37,6 +40,9 @@ struct Sched {
     int n_full;  // tiles with a single item
     int k, zc;   // chunks per remaining tile, planes per chunk
     int nty;     // tiles along y
+    int za;      // 0, or the "split" list for grids with about as many tiles as SMs: EVERY tile is cut at stored plane za;
+                 // item b < tiles is tile b over planes [0, za), item tiles + b is tile b over [za, nz).  The long items
+                 // are dispatched first, the short ones fill the SMs that would otherwise idle (n_full, k, zc unused).
     int ov;      // 0, or (include/fd6_testing.h, fd_debug_set_tile_overlap) the number of values by which neighbouring tiles
                  // overlap in x and y: every tile is still computed in full, a value is stored by the tile that holds it
                  // furthest from its edge.  Emulates the redundant halo-ring evaluation of temporal blocking (DESIGN 7).
@@ -177,16 +183,33 @@ inline int tiled_make_map(TiledState& ts, CUtensorMap* tm, void* base, long long
 // Work list (see Sched; pure host arithmetic, also reachable through fd_plan_work_list for the CPU tests): one CTA
 // per SM is resident, so whole waves of S tiles run as full columns and the remaining tiles are cut into the
 // number of z-chunks that minimises (waves x planes staged per item).
+// Time (in planes) at which a launch ends when its items, `count[i]` items of `cost[i]` planes each in this order, are
+// dispatched in index order, each to the SM that becomes free first (one resident CTA per SM): what the hardware does.
+inline long long list_makespan(const int* count, const int* cost, int classes, int S) {
+    std::priority_queue<long long, std::vector<long long>, std::greater<long long>> free_at;
+    for (int s = 0; s < S; ++s) free_at.push(0);
+    long long end = 0;
+    for (int c = 0; c < classes; ++c)
+        for (int i = 0; i < count[c]; ++i) {
+            const long long t = free_at.top() + cost[c];
+            free_at.pop();
+            free_at.push(t);
+            end = std::max(end, t);
+        }
+    return end;
+}
+
 inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     const int tiles = ntx * nty;
     const int n_full = (tiles / S) * S, rem = tiles - n_full;
+    const int warm = 2 * R + 4;  // planes an item stages before its first output (+ fill latency)
     int best_k = 1;
     double best_cost = 1e300;
     for (int k = 1; rem > 0 && k <= (nz + 1) / 2 && k <= 64; ++k) {  // chunks of >= 2 planes
         const int zc = (nz + k - 1) / k;
         const int real = (nz + zc - 1) / zc;
         const long long waves = ((long long)rem * real + S - 1) / S;
-        const double cost = (double)waves * (zc + 2 * R + 4);  // time ~ waves x planes staged per item (+ fill latency)
+        const double cost = (double)waves * (zc + warm);  // time ~ waves x planes staged per item
         if (cost < best_cost) {
             best_cost = cost;
             best_k = k;
@@ -196,10 +219,41 @@ inline Sched plan_work_list(int ntx, int nty, int nz, int S, int* items) {
     sc.ntx = ntx;
     sc.nty = nty;
     sc.ov = 0;
+    sc.za = 0;
     sc.n_full = n_full;
     sc.zc = (nz + best_k - 1) / best_k;
     sc.k = (nz + sc.zc - 1) / sc.zc;
     *items = n_full + rem * sc.k;
+    // Grids with about as many tiles as SMs (C3: 128 tall tiles on 148 SMs) leave SMs idle for a whole column, and cutting
+    // only a remainder cannot help while any item is a full column.  Cut EVERY tile at one plane za instead: the long
+    // parts go out first, the short parts are packed onto the SMs left over (C3: 128 x 232 planes + 128 x 24 planes,
+    // the launch ends after 242 plane-times instead of 266 by this model).  Taken when the model beats the two-tier list by
+    // more than 3 %.  Measured at C3 in one session (profiles/r03_alt_split_C3_*.json.txt): first repetition 13092 ->
+    // 13626 Mcell/s (+4 %, less than the model's 9 %: a short item costs more than its planes + warm-up), median of five
+    // under the rising power cap 12203 / 12585 -> 12648; a cut 8 planes lower (224) is 4 % SLOWER than no split, so the
+    // plane comes from the model's minimum, never from a round number.
+    if (tiles < 4 * S && nz >= 16) {
+        const int cnt2[2] = {n_full, rem * sc.k}, cost2[2] = {nz + warm, sc.zc + warm};
+        const long long cur = list_makespan(cnt2, cost2, 2, S);
+        long long best = cur;
+        int best_za = 0;
+        const int step = std::max(1, nz / 256);
+        for (int za = (nz + 1) / 2; za <= nz - 2; za += step) {
+            const int cnt[2] = {tiles, tiles}, cost[2] = {za + warm, nz - za + warm};
+            const long long m = list_makespan(cnt, cost, 2, S);
+            if (m < best) {
+                best = m;
+                best_za = za;
+            }
+        }
+        if (best_za > 0 && 100 * best < 97 * cur) {
+            sc.za = best_za;
+            sc.n_full = 0;
+            sc.k = 2;
+            sc.zc = best_za;
+            *items = 2 * tiles;
+        }
+    }
     return sc;
 }
 

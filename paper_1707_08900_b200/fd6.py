@@ -48,7 +48,7 @@ class FdInfo(C.Structure):
 
 class FdWorkList(C.Structure):
     _fields_ = [(n, C.c_int) for n in ("tile_x", "tile_y", "tiles_x", "tiles_y", "planes", "full_tiles", "chunks",
-                                       "chunk_planes", "items")]
+                                       "chunk_planes", "items", "split_plane")]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p, C.c_void_p)

@@ -132,8 +132,11 @@ def test_no_cpu_fallback_without_a_device(fd6):
 
 def _items(wl):
     """Enumerate (tile, plane range) of every launch-grid item exactly as fd6.h documents it."""
+    tiles = wl.tiles_x * wl.tiles_y
     for b in range(wl.items):
-        if b < wl.full_tiles:
+        if wl.split_plane > 0:
+            yield (b, 0, wl.split_plane) if b < tiles else (b - tiles, wl.split_plane, wl.planes)
+        elif b < wl.full_tiles:
             yield b, 0, wl.planes
         else:
             j = b - wl.full_tiles
@@ -153,8 +156,11 @@ def test_work_list_covers_every_tile_plane_exactly_once(fd6, shape, dtype, sms):
     assert wl.tiles_y * wl.tile_y >= ny > (wl.tiles_y - 1) * wl.tile_y
     paired = dtype == 0 and nz % 2 == 0
     assert wl.planes == (nz // 2 if paired else nz)
-    assert wl.full_tiles % sms == 0 and 0 <= tiles - wl.full_tiles < sms
-    assert wl.items == wl.full_tiles + (tiles - wl.full_tiles) * wl.chunks
+    if wl.split_plane > 0:  # every tile cut once, the long part first
+        assert wl.items == 2 * tiles and wl.full_tiles == 0 and wl.planes / 2 <= wl.split_plane <= wl.planes - 2
+    else:
+        assert wl.full_tiles % sms == 0 and 0 <= tiles - wl.full_tiles < sms
+        assert wl.items == wl.full_tiles + (tiles - wl.full_tiles) * wl.chunks
     covered = [0] * (tiles * wl.planes)
     for tile, zs, ze in _items(wl):
         assert 0 <= tile < tiles
@@ -174,6 +180,11 @@ def test_work_list_of_the_headline_config(fd6):
     assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes) == (32, 12, 4, 11, 64)
     wl = fd6.fd_plan_work_list(256, 256, 256, fd6.FD_F64, 148)
     assert (wl.tile_x, wl.tile_y, wl.tiles_x, wl.tiles_y, wl.planes) == (32, 16, 8, 16, 256)
+    # C3: 128 tiles on 148 SMs.  Full columns would leave 20 SMs idle for the whole launch (266 plane-times with the
+    # warm-up); the split list gives every SM work: 128 long parts, and the 128 short parts packed 6-7 deep on 20 SMs
+    assert wl.split_plane > 0 and wl.items == 256 and wl.full_tiles == 0
+    long_cost, short_cost = wl.split_plane + 10, wl.planes - wl.split_plane + 10
+    assert max(long_cost, 7 * short_cost) <= 245
 
 
 def test_work_list_cuts_thin_grids_into_short_chunks(fd6):
