@@ -336,10 +336,12 @@ static int launch_substep(fd_ctx* c, const SubD& sd) {
         if constexpr (std::is_same<T, float>::value) {  // plain fp32: two x-adjacent cells per thread
             dim3 grid2((g.nx + 127) / 128, band_rows, bands * g.nz);
             k_direct_pass2_x2<<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s);
-        } else if (tiled && g.nx >= 128) {
-            // staged variants on rows wide enough to fill the block: value pairs, z-marching (the seven div planes of the
-            // z derivative stay in registers, so no y banding is needed to keep them in L2)
-            const int zc = 16;  // planes per thread: 6 warm-up div loads per 16 planes, 16 chunk layers at C4
+        } else if (const int zc = 16;  // planes per thread: 6 warm-up div loads per 16 planes, 16 chunk layers at C4
+                   tiled && g.nx >= 128 &&
+                   (long long)((g.nx + 127) / 128) * ((g.ny + 3) / 4) * ((g.nz + zc - 1) / zc) >= 4LL * std::max(c->tiled.sm_count, 1)) {
+            // staged variants on rows wide enough to fill the block and grids that give every SM several blocks (C2's 128
+            // blocks would not: 11887 -> 11264 Mcell/s, it keeps the kernel below): value pairs, z-marching (the seven div
+            // planes of the z derivative stay in registers, so no y banding is needed to keep them in L2)
             dim3 grid2((g.nx + 127) / 128, (g.ny + 3) / 4, (g.nz + zc - 1) / zc);
             if (s.write_w)
                 k_pass2_march<T, true><<<grid2, block, 0, c->stream>>>(Div, Fout, W, g, k, s, zc);
