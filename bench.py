@@ -423,6 +423,8 @@ def main():
     step_gbs_actual = WORDS_PER_CELL_STEP_ACTUAL[args.path] * esize * N * K / (ms_max * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": (achieved / peak if achieved else None),
+                "frac_is": (f"contract figure: {words} words per cell and launch (SURVEY 8(d)); averaged over the three substeps a "
+                            f"launch moves {DOMINANT_WORDS_ACTUAL_MEAN[args.path]:.1f} (w skipped on substeps 1 and 3): frac_actual_bytes"),
                 "frac_nominal": (achieved / NOMINAL_HBM_GBS if achieved else None),
                 # the same launches counted with the bytes they really move (w skipped on substeps 1 and 3)
                 "achieved_actual_bytes": actual, "frac_actual_bytes": (actual / peak if actual else None),

@@ -388,6 +388,28 @@ def test_error_codes_on_a_live_context(mods):
     ctx.fd_destroy()
 
 
+def test_fd_get_info_reports_what_the_context_launches(mods):
+    """variant, prepared tile shape, tile extents and work items come from the context, not from a planner call."""
+    O, fd6, I = mods
+    ctx = fd6.Fd(32, 32, 32, 0.1, 0.01, 1.0, fd6.FD_F64)  # AUTO on a tiny grid: the one-thread-per-cell kernels
+    info = ctx.fd_get_info()
+    assert info.variant == fd6.FD_VARIANT_DIRECT and (info.tile_shape, info.tile_x, info.tile_y, info.work_items) == (-1, 0, 0, 0)
+    assert info.graph_state == fd6.FD_GRAPH_WAITING and info.graph_note == b""
+    ctx.fd_set_graphs(False)
+    assert ctx.fd_get_info().graph_state == fd6.FD_GRAPH_OFF
+    ctx.fd_destroy()
+    sms = __import__("torch").cuda.get_device_properties(0).multi_processor_count
+    ctx = fd6.Fd(256, 256, 64, 0.1, 0.01, 1.0, fd6.FD_F64)  # 8 x 16 tall tiles
+    info = ctx.fd_get_info()
+    wl = fd6.fd_plan_work_list(256, 256, 64, fd6.FD_F64, sms)
+    assert info.variant == fd6.FD_VARIANT_TILED and (info.tile_shape, info.tile_x, info.tile_y) == (1, 32, 16)
+    assert info.work_items == wl.items and (wl.split_plane > 0) == (wl.items == 2 * wl.tiles_x * wl.tiles_y)
+    ctx.fd_set_tile_shape(0)
+    info = ctx.fd_get_info()
+    assert (info.tile_shape, info.tile_x, info.tile_y) == (0, 32, 12) and info.work_items > 0
+    ctx.fd_destroy()
+
+
 def test_profile_counters_count_the_launches(mods):
     O, fd6, I = mods
     ctx = fd6.Fd(64, 64, 64, 0.1, 0.01, 1.0, fd6.FD_F32)
